@@ -1,0 +1,5 @@
+"""Float64 CPU oracle of the LLOID hot path -- test infrastructure only (see lloid_oracle.py header)."""
+from .lloid_oracle import (  # noqa: F401
+    N_DOWN, N_UP, Series, resample_kernel, decimate, upsample, upsample_input_range,
+    basis_correlate, reconstruct, rate_groups, lloid_snr, brute_force, find_peaks,
+)
