@@ -1,0 +1,126 @@
+/* lloid.h -- C ABI of the B200-native LLOID multirate SVD matched-filter hot path.
+ *
+ * The operations are those of arxiv/paper_2511_04730 (SGNL), Sec. II.C-II.D.1; citations are
+ * /root/reference/PAPER.md:<line>.  Symbols follow the paper: f0 strain rate, slice s with rate f^s,
+ * N^s taps, L^s orthonormal basis filters u_l^s (Eq. 3), reconstruction matrix
+ * sigma_l nu_il (Eq. 6), M complex templates = 2M real rows.
+ *
+ * One push of a strain buffer runs, entirely in CUDA kernels on the caller's stream:
+ *   a1 decimate   d_r[j] = sqrt(D) sum_k ghat_D[k] d[jD + c - k], c = n_down*D      (Eq. 4)
+ *   a2 correlate  Y^s[l,j] = sum_n u_l^s[n] d_{f^s}[j - delay_s - N^s + 1 + n]     (Eq. 5; Eq. 9, 167-185)
+ *   a3 reconstruct + a4 combine   rho = sum_s Up(...Up(R^s Y^s))                    (Eqs. 6-9, Fig. 4)
+ *   a5 peaks      per template j: first k maximising rho_2j[k]^2 + rho_2j+1[k]^2
+ * SNR sample k of a push is stream sample n0+k (n0 = samples pushed before); it reads strain <= n0+k only.
+ *
+ * All pointers are plain host or device pointers as stated per argument; no C++/torch types cross this
+ * boundary.  Every function returns 0 (LLOID_OK) or a negative lloid_status; on failure nothing is changed
+ * and lloid_last_error() (thread-local) describes the reason.  There is no CPU fallback: every call that
+ * computes needs a CUDA device of compute capability 10.0 (sm_100a).
+ */
+#ifndef LLOID_H_
+#define LLOID_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+  LLOID_OK = 0,
+  LLOID_EINVAL = -1,   /* null pointer, bad size, rate not a power-of-two divisor of f0, rates increasing with s,
+                          slices that do not abut, delay[0] != 0, buffer_len not a multiple of max D_s */
+  LLOID_ELATENCY = -2, /* a slice with f^s < f0 whose delay is shorter than the look-ahead of its decimator and
+                          upsample chain: delay_s < n_down + H_g (PAPER.md:161-163 causality condition) */
+  LLOID_ENOMEM = -3,   /* host or device allocation failed */
+  LLOID_ECUDA = -4,    /* a CUDA runtime/driver call failed, or the device is not sm_100 */
+  LLOID_ESTATE = -5    /* call not valid in this state (e.g. debug_bank out of range) */
+} lloid_status;
+
+typedef enum {
+  LLOID_PREC_FP32_FFMA = 0, /* every contraction in fp32 on the CUDA cores (gate 1e-4 of SNR rms)              */
+  LLOID_PREC_F16 = 1,       /* tcgen05 kind::f16, operands rounded once to fp16, fp32 accumulate in TMEM         */
+  LLOID_PREC_F16_SPLIT = 2  /* tcgen05 kind::f16, every operand split hi+lo fp16, 3 MMAs per product (default)  */
+} lloid_precision;
+
+/* One time slice of an SVD bank.  Arrays may be host or device memory; create copies them. */
+typedef struct {
+  int32_t rate_hz;     /* f^s: power of two, divides strain_rate_hz, non-increasing with s, rate_hz[0] = f0  */
+  int32_t n_taps;      /* N^s, samples at rate_hz                                                            */
+  int32_t n_basis;     /* L^s >= 1                                                                           */
+  int64_t delay;       /* t^s * rate_hz: samples (at rate_hz) between the merger and this slice's newest tap;
+                          delay[0] = 0; slices abut: (delay_s + n_taps_s)/rate_s = delay_{s+1}/rate_{s+1}     */
+  const float *basis;  /* U^s [n_basis][n_taps] row-major, orthonormal rows, oldest tap first                 */
+  const float *recon;  /* R^s [2*M][n_basis] row-major = V diag(sigma); row 2j = real, 2j+1 = imaginary part  */
+} lloid_slice;
+
+/* Per-template, per-buffer trigger (time, SNR, phase; integer sample). */
+typedef struct {
+  float snr;           /* max_k |rho_2j[k] + i rho_2j+1[k]| over the pushed buffer                            */
+  int32_t sample;      /* first k in [0, buffer_len) attaining it (-1 if below options.threshold)            */
+  float phase;         /* atan2(rho_2j+1[k], rho_2j[k]) at that k                                             */
+} lloid_peak;
+
+typedef struct {
+  int32_t n_down;      /* decimator half length in output samples; default 32                  */
+  int32_t n_up;        /* upsampler half length in input samples; default 8 (only 8 supported) */
+  int32_t precision;   /* lloid_precision; default LLOID_PREC_F16_SPLIT                                      */
+  float threshold;     /* report only peaks with snr >= threshold; 0 = report every template's peak          */
+} lloid_options;
+
+typedef struct lloid_bank lloid_bank;      /* opaque, immutable after create; owns host+device copies of U, R */
+typedef struct lloid_stream lloid_stream;  /* opaque; owns the device rings / state of (banks x detectors)    */
+
+/* Fill *opt with the defaults above. */
+void lloid_options_default(lloid_options *opt);
+
+/* Build one SVD bank of M complex templates from its slice table ("during
+ * initialization").  `slices[s].basis/recon` may be host or device pointers and may be freed on return.
+ * opt == NULL means defaults.  Errors: EINVAL, ELATENCY, ENOMEM, ECUDA. */
+int lloid_bank_create(lloid_bank **out, int32_t strain_rate_hz, int32_t n_templates, int32_t n_slices,
+                      const lloid_slice *slices, const lloid_options *opt);
+void lloid_bank_destroy(lloid_bank *bank);
+
+/* A stream filters n_detectors independent strain series against every bank (same banks for all
+ * detectors: flat-PSD synthetic case; per-detector banks = one stream per detector).
+ * buffer_len (f0 samples per push) must be a multiple of every bank's largest decimation factor.
+ * cuda_stream is a cudaStream_t (NULL = legacy default stream); all work of push/reset is enqueued on it.
+ * All banks must use the same precision and must outlive the stream. */
+int lloid_stream_create(lloid_stream **out, const lloid_bank *const *banks, int32_t n_banks,
+                        int32_t n_detectors, int32_t buffer_len, void *cuda_stream);
+void lloid_stream_destroy(lloid_stream *stream);
+
+/* Push one buffer.  Asynchronous on the stream's cuda_stream; no host synchronisation inside.
+ *   strain     DEVICE, [n_detectors][buffer_len] fp32 whitened strain (gaps = zeros)
+ *   peaks      DEVICE, [n_detectors][sum_b M_b] lloid_peak, banks in creation order
+ *   snr_debug  DEVICE or NULL: [n_detectors][2*M_debug][buffer_len] fp32, the full SNR series of bank
+ *              `debug_bank` (row 2j real, 2j+1 imaginary).  NULL in production: SNR never reaches HBM.
+ * Buffers are caller-owned and must stay valid until the stream reaches the end of this push. */
+int lloid_stream_push(lloid_stream *stream, const float *strain, lloid_peak *peaks, float *snr_debug,
+                      int32_t debug_bank);
+
+/* Same through HOST buffers: copies strain host->device, pushes, copies peaks device->host and waits for
+ * the stream.  strain_host [n_detectors][buffer_len], peaks_host [n_detectors][sum_b M_b]; pinned memory
+ * makes the copies asynchronous but is not required. */
+int lloid_stream_push_host(lloid_stream *stream, const float *strain_host, lloid_peak *peaks_host);
+
+/* Zero all rings and the stream clock: the next push is stream sample 0 (zero history). */
+int lloid_state_reset(lloid_stream *stream);
+
+/* Introspection (host values, no device work). */
+int64_t lloid_stream_samples_pushed(const lloid_stream *stream);
+int32_t lloid_stream_total_templates(const lloid_stream *stream);
+int32_t lloid_stream_launches_per_push(const lloid_stream *stream); /* kernels this library launches per push */
+/* Executed and algorithmic work of one push, for roofline accounting:
+ * out[0] a2 flop executed, out[1] a3 flop executed, out[2] a2 algorithmic flop (2 sum L N f),
+ * out[3] a3+a4 algorithmic flop in the paper's order (2 sum 2M L f + 16*2M*sum f_out),
+ * out[4] bytes of operands (U, R) one push reads, out[5] bytes of Y/Yup intermediates written+read. */
+int lloid_stream_work_per_push(const lloid_stream *stream, double out[6]);
+
+const char *lloid_last_error(void);
+const char *lloid_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LLOID_H_ */

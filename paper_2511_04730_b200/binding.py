@@ -1,0 +1,241 @@
+"""Thin ctypes binding of liblloid.so (include/lloid.h): argument marshalling only.
+
+Every step of the hot path runs in the library's CUDA kernels; PyTorch is used here for device memory and
+streams.  There is no CPU fallback: importing this module without the built library raises.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from typing import List, Optional, Sequence
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblloid.so")
+
+LLOID_OK, LLOID_EINVAL, LLOID_ELATENCY, LLOID_ENOMEM, LLOID_ECUDA, LLOID_ESTATE = 0, -1, -2, -3, -4, -5
+LLOID_PREC_FP32_FFMA, LLOID_PREC_F16, LLOID_PREC_F16_SPLIT = 0, 1, 2
+
+PEAK_DTYPE = np.dtype([("snr", np.float32), ("sample", np.int32), ("phase", np.float32)])
+
+
+class lloid_slice(C.Structure):
+    _fields_ = [("rate_hz", C.c_int32), ("n_taps", C.c_int32), ("n_basis", C.c_int32), ("delay", C.c_int64),
+                ("basis", C.c_void_p), ("recon", C.c_void_p)]
+
+
+class lloid_options(C.Structure):
+    _fields_ = [("n_down", C.c_int32), ("n_up", C.c_int32), ("precision", C.c_int32), ("threshold", C.c_float)]
+
+
+class LloidError(RuntimeError):
+    def __init__(self, code: int, msg: str):
+        super().__init__(f"lloid error {code}: {msg}")
+        self.code = code
+
+
+def _load():
+    if not os.path.exists(LIB_PATH):
+        raise ImportError(f"{LIB_PATH} is missing: run `python paper_2511_04730_b200/build.py` "
+                          "(there is no CPU fallback)")
+    lib = C.CDLL(LIB_PATH)
+    vp, i32, i64 = C.c_void_p, C.c_int32, C.c_int64
+    sig = {
+        "lloid_options_default": (None, [C.POINTER(lloid_options)]),
+        "lloid_bank_create": (C.c_int, [C.POINTER(vp), i32, i32, i32, C.POINTER(lloid_slice), C.POINTER(lloid_options)]),
+        "lloid_bank_destroy": (None, [vp]),
+        "lloid_stream_create": (C.c_int, [C.POINTER(vp), C.POINTER(vp), i32, i32, i32, vp]),
+        "lloid_stream_destroy": (None, [vp]),
+        "lloid_stream_push": (C.c_int, [vp, vp, vp, vp, i32]),
+        "lloid_stream_push_host": (C.c_int, [vp, vp, vp]),
+        "lloid_state_reset": (C.c_int, [vp]),
+        "lloid_stream_samples_pushed": (i64, [vp]),
+        "lloid_stream_total_templates": (i32, [vp]),
+        "lloid_stream_launches_per_push": (i32, [vp]),
+        "lloid_stream_work_per_push": (C.c_int, [vp, C.POINTER(C.c_double)]),
+        "lloid_last_error": (C.c_char_p, []),
+        "lloid_version": (C.c_char_p, []),
+    }
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
+    return lib
+
+
+_lib = _load()
+EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_state_reset",
+           "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
+           "lloid_stream_work_per_push", "lloid_last_error", "lloid_version"]
+
+
+def lloid_last_error() -> str:
+    return _lib.lloid_last_error().decode()
+
+
+def lloid_version() -> str:
+    return _lib.lloid_version().decode()
+
+
+def _check(rc: int):
+    if rc != LLOID_OK:
+        raise LloidError(rc, lloid_last_error())
+
+
+def lloid_options_default() -> lloid_options:
+    o = lloid_options()
+    _lib.lloid_options_default(C.byref(o))
+    return o
+
+
+def lloid_bank_create(strain_rate_hz: int, n_templates: int, slices: Sequence[dict], precision: Optional[int] = None,
+                      threshold: float = 0.0, n_down: int = 32) -> int:
+    """slices: dicts with rate_hz, n_taps, n_basis, delay, basis (float32 [L][N]), recon (float32 [2M][L]);
+    arrays are contiguous numpy arrays (host) or torch CUDA tensors (device).  Returns the bank handle."""
+    arr = (lloid_slice * len(slices))()
+    keep = []
+    for i, s in enumerate(slices):
+        ptrs = []
+        for key in ("basis", "recon"):
+            a = s[key]
+            if isinstance(a, np.ndarray):
+                a = np.ascontiguousarray(a, dtype=np.float32)
+                ptrs.append(a.ctypes.data)
+            else:   # torch tensor
+                a = a.contiguous().float()
+                ptrs.append(a.data_ptr())
+            keep.append(a)
+        arr[i] = lloid_slice(int(s["rate_hz"]), int(s["n_taps"]), int(s["n_basis"]), int(s["delay"]), ptrs[0], ptrs[1])
+    opt = lloid_options_default()
+    opt.n_down = n_down
+    opt.threshold = threshold
+    if precision is not None:
+        opt.precision = precision
+    h = C.c_void_p()
+    _check(_lib.lloid_bank_create(C.byref(h), strain_rate_hz, n_templates, len(slices), arr, C.byref(opt)))
+    return h.value
+
+
+def lloid_bank_destroy(bank: int):
+    _lib.lloid_bank_destroy(bank)
+
+
+def lloid_stream_create(banks: Sequence[int], n_detectors: int, buffer_len: int, cuda_stream: int = 0) -> int:
+    arr = (C.c_void_p * len(banks))(*banks)
+    h = C.c_void_p()
+    _check(_lib.lloid_stream_create(C.byref(h), arr, len(banks), n_detectors, buffer_len, cuda_stream))
+    return h.value
+
+
+def lloid_stream_destroy(stream: int):
+    _lib.lloid_stream_destroy(stream)
+
+
+def lloid_stream_push(stream: int, strain_ptr: int, peaks_ptr: int, snr_debug_ptr: int = 0, debug_bank: int = 0):
+    """Raw device pointers (torch tensors' data_ptr())."""
+    _check(_lib.lloid_stream_push(stream, strain_ptr, peaks_ptr, snr_debug_ptr or None, debug_bank))
+
+
+def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):
+    _check(_lib.lloid_stream_push_host(stream, strain_host_ptr, peaks_host_ptr))
+
+
+def lloid_state_reset(stream: int):
+    _check(_lib.lloid_state_reset(stream))
+
+
+def lloid_stream_samples_pushed(stream: int) -> int:
+    return _lib.lloid_stream_samples_pushed(stream)
+
+
+def lloid_stream_total_templates(stream: int) -> int:
+    return _lib.lloid_stream_total_templates(stream)
+
+
+def lloid_stream_launches_per_push(stream: int) -> int:
+    return _lib.lloid_stream_launches_per_push(stream)
+
+
+def lloid_stream_work_per_push(stream: int) -> List[float]:
+    out = (C.c_double * 6)()
+    _check(_lib.lloid_stream_work_per_push(stream, out))
+    return list(out)
+
+
+# ---------------------------------------------------------------------------------------------------
+# convenience wrappers (still marshalling only)
+# ---------------------------------------------------------------------------------------------------
+def bank_slices(bank) -> List[dict]:
+    """Slice table of a workloads.Bank-like object (attributes f0, M, slices[*].rate/n_taps/delay/U/R)."""
+    return [dict(rate_hz=s.rate, n_taps=s.n_taps, n_basis=s.U.shape[0], delay=s.delay,
+                 basis=np.ascontiguousarray(s.U, dtype=np.float32), recon=np.ascontiguousarray(s.R, dtype=np.float32))
+            for s in bank.slices]
+
+
+class LloidStream:
+    """Owns bank and stream handles plus the torch device buffers a push needs."""
+
+    def __init__(self, banks, n_detectors: int, buffer_len: int, precision: int = LLOID_PREC_F16_SPLIT,
+                 threshold: float = 0.0, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("LloidStream needs a CUDA device (no CPU fallback)")
+        self.torch = torch
+        self.device = torch.device(device)
+        torch.cuda.set_device(self.device)
+        self.n_det, self.B = n_detectors, buffer_len
+        self.Ms = [b.M for b in banks]
+        self.bank_handles = [lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold) for b in banks]
+        self.cuda_stream = torch.cuda.current_stream(self.device)
+        self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
+        self.Mtot = lloid_stream_total_templates(self.handle)
+        self.peaks_dev = torch.zeros((n_detectors, self.Mtot, 3), dtype=torch.int32, device=self.device)
+        self.strain_dev = torch.zeros((n_detectors, buffer_len), dtype=torch.float32, device=self.device)
+        self.peaks_host = torch.zeros((n_detectors, self.Mtot, 3), dtype=torch.int32).pin_memory()
+        self.strain_host = torch.zeros((n_detectors, buffer_len), dtype=torch.float32).pin_memory()
+
+    def push_device(self, strain_dev, snr_debug=None, debug_bank: int = 0):
+        """strain_dev: CUDA float32 [n_det][B]; asynchronous.  Returns the device peaks tensor (int32 view)."""
+        assert strain_dev.is_cuda and strain_dev.dtype == self.torch.float32 and strain_dev.is_contiguous()
+        assert tuple(strain_dev.shape) == (self.n_det, self.B)
+        lloid_stream_push(self.handle, strain_dev.data_ptr(), self.peaks_dev.data_ptr(),
+                          0 if snr_debug is None else snr_debug.data_ptr(), debug_bank)
+        return self.peaks_dev
+
+    def push(self, strain: np.ndarray, want_snr_bank: Optional[int] = None):
+        """Host numpy [n_det][B] in, structured peaks [n_det][Mtot] out (and SNR [n_det][2M][B] if asked)."""
+        t = self.torch
+        self.strain_dev.copy_(t.from_numpy(np.ascontiguousarray(strain, dtype=np.float32)))
+        snr = None
+        if want_snr_bank is not None:
+            snr = t.zeros((self.n_det, 2 * self.Ms[want_snr_bank], self.B), dtype=t.float32, device=self.device)
+        self.push_device(self.strain_dev, snr, want_snr_bank or 0)
+        t.cuda.synchronize(self.device)
+        peaks = self.peaks_dev.cpu().numpy().view(PEAK_DTYPE).reshape(self.n_det, self.Mtot)
+        return (peaks, snr.cpu().numpy()) if snr is not None else peaks
+
+    def push_host(self):
+        """End-to-end call on the pinned host buffers self.strain_host -> self.peaks_host (synchronous)."""
+        lloid_stream_push_host(self.handle, self.strain_host.data_ptr(), self.peaks_host.data_ptr())
+        return self.peaks_host.numpy().view(PEAK_DTYPE).reshape(self.n_det, self.Mtot)
+
+    def reset(self):
+        lloid_state_reset(self.handle)
+
+    def work_per_push(self):
+        return lloid_stream_work_per_push(self.handle)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            lloid_stream_destroy(self.handle)
+            self.handle = None
+        for b in getattr(self, "bank_handles", []):
+            lloid_bank_destroy(b)
+        self.bank_handles = []
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

@@ -1,0 +1,120 @@
+// Internal declarations shared by the host code and the kernels of liblloid (not part of the C ABI).
+// Notation follows include/lloid.h and DESIGN.md: f0, D = f0/rate, N taps, L bases, delay, group g =
+// run of slices at one rate, A_g/H_g = low/high halo (in samples at the group's rate) of the zero-phase
+// upsample chain above the group (Eqs. 7-9).
+#pragma once
+#include <cuda_fp16.h>
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "../../include/lloid.h"
+
+#define LLOID_MAX_GROUPS 12   // distinct rates in one bank (2048 .. 1 Hz)
+#define LLOID_MAX_RATES 12    // distinct rates in one stream
+#define LLOID_NUP 8
+
+namespace lloid {
+
+void set_error(const char *fmt, ...);
+
+// ---------------------------------------------------------------------------------------------- bank
+struct SliceInfo {
+  int rate, D, N, L, group, koff;   // koff: first column of this slice in the bank's concatenated K axis
+  long long delay;
+  std::vector<float> U;              // host copy [L][N]; stacked per geometry class at stream_create
+};
+struct GroupInfo {
+  int rate, D, f;                    // f = rate_{g-1}/rate_g (1 for g = 0)
+  int A, H;                          // columns [n0/D - A, (n0+B)/D + H) of this group feed one push
+  int first_slice, n_slices;
+};
+}  // namespace lloid
+
+struct lloid_bank {
+  int f0, M, Mpad, S, G;
+  lloid_options opt;
+  std::vector<lloid::SliceInfo> slices;
+  std::vector<lloid::GroupInfo> groups;
+  int Ktot, Kpad;                    // sum_s L^s and its round-up to 64
+  float r_scale;                     // power of two applied to R before the fp16 cast (1 for fp32)
+  float *dR32;                       // FFMA:   [2 (re,im)][Mpad][Kpad] fp32
+  __half *dR16;                      // tensor: [planes (hi,lo)][2 (re,im)][Mpad][Kpad] fp16, scaled by r_scale
+  int r_planes;
+};
+
+// ---------------------------------------------------------------------------------------------- device tables
+namespace lloid {
+
+struct RateDev {                     // one per distinct rate in the stream (index 0 = f0)
+  float *ring2;                      // [n_det][2*rlen] mirrored ring of the strain decimated to this rate
+  const float *taps;                 // sqrt(D)*ghat_D[k], k = 0..2c  (Eq. 4), nullptr for D = 1
+  int D, rlen, lag, c;               // ring slot of sample j is (j + lag) mod rlen; lag = n_down (0 for D = 1)
+  int out_begin;                     // first flattened decimator output index of this rate in a push
+  int n_out;                         // B / D
+};
+
+struct DecimParams {
+  RateDev r[LLOID_MAX_RATES];
+  int n_rates, n_det, B, total_out, copy_blocks;
+};
+
+struct CorrClass {                   // slices (across banks) with identical (rate, N, delay, H): stacked U
+  const float *ring2;                // rate ring, detector 0
+  long long ring_det_stride;
+  int rlen, lag, D, N, Npad, H;
+  long long delay;
+  int Lstack, Lpad;                  // stacked basis rows and their round-up to 128
+  const float *U32;                  // [Lpad][Npad] fp32 (FFMA path)
+  const __half *U16;                 // [planes][Lpad][Npad] fp16 scaled by u_scale (tensor path)
+  float *yring;                      // [n_det][ylen][Lpad] fp32 ring of Y columns; slot of column j = (j + 64) mod ylen
+  long long ydet_stride;
+  int ylen, ncols;                   // ncols = B / D new columns per push: [n0/D + H, (n0+B)/D + H)
+  float u_scale_inv;
+};
+
+struct CorrTile { int cls, row0, col0; };   // FFMA a2 work item: 64 rows x 64 columns
+
+struct UpItem {                      // one (bank, slice, chunk of <=32 basis rows)
+  const float *yring; long long ydet_stride; int ylen, ypitch, row0, nl;
+  int kcol;                          // first column in the bank's Yup (koff_s + chunk*32)
+  int g;                             // group of the slice = number of upsample stages
+  int log2f[LLOID_MAX_GROUPS];       // log2 f_h of stage h -> h-1, h = 1..g
+  int D;                             // D of the slice's group
+  void *yup; long long yup_det_stride, yup_plane_stride; int kpitch;
+};
+
+struct ReconBank {                   // a3 work description of one bank
+  const float *R32; const __half *R16; long long r_part_stride, r_plane_stride;
+  const void *yup; long long yup_det_stride, yup_plane_stride;
+  int M, Mpad, Kpad, tmpl_off;       // tmpl_off: first template of this bank in the stream's peak array
+  float inv_scale2;                  // 1/(r_scale^2): applied to |z|^2
+  float inv_scale;
+};
+
+struct PeakPartial { float p; int idx; float re, im; };
+
+// ---------------------------------------------------------------------------------------------- launchers (kernels_*.cu)
+cudaError_t launch_decimate(const DecimParams &P, const float *strain, const long long *n0, cudaStream_t st);
+cudaError_t launch_corr_ffma(const CorrClass *cls_dev, const CorrTile *tiles_dev, int n_tiles, int n_det,
+                             const long long *n0, cudaStream_t st);
+cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
+                            const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st);
+cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
+                              PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
+cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
+                            lloid_peak *peaks, long long *n0, int B, cudaStream_t st);
+
+// ---------------------------------------------------------------------------------------------- tcgen05 path (kernels_tc.cu)
+struct TcPlan;
+int tc_time_splits(int B);   // partial peaks per template written by the tensor-core a3 kernel
+int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
+                   const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes);
+void tc_plan_destroy(TcPlan *p);
+cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st);
+cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank,
+                            cudaStream_t st);
+
+}  // namespace lloid

@@ -1,0 +1,336 @@
+// lloid_stream_*: device-resident streaming state (per-rate strain rings, per-class Y rings), the stacking of
+// equal-geometry slices across banks ("multidimensional filtering"), and the per-push launch
+// sequence  K1 decimate -> a2 correlate -> K_up upsample -> a3 reconstruct+peaks -> finalize.
+#include <algorithm>
+#include <cmath>
+#include <cstring>
+#include <map>
+#include <new>
+#include <tuple>
+
+#include "lloid_internal.h"
+
+using namespace lloid;
+
+struct lloid_stream {
+  std::vector<const lloid_bank *> banks;
+  int n_det, B, f0, precision, n_down, Mtot, n_tt, max_mtiles;
+  float threshold;
+  cudaStream_t st;
+  long long n0_host;
+  long long *n0_dev;
+  DecimParams dec;
+  std::vector<CorrClass> classes;
+  CorrClass *classes_dev;
+  CorrTile *tiles_dev; int n_tiles;
+  UpItem *items_dev; int n_items;
+  float *uptaps_dev; int *uptap_off_dev;
+  ReconBank *rbanks_dev;
+  std::vector<ReconBank> rbanks;
+  PeakPartial *partial_dev;
+  float *strain_dev; lloid_peak *peaks_dev;       // staging for push_host
+  std::vector<void *> allocs;                      // every cudaMalloc of this stream
+  std::vector<std::pair<void *, size_t>> state;    // (ptr, bytes) zeroed by reset
+  int up_planes, up_chunk;
+  double work[6];
+  TcPlan *tc;                                      // tensor-core launch plan (kernels_tc.cu), nullptr for FFMA
+};
+
+static double sinc_pi(double x) { return x == 0.0 ? 1.0 : std::sin(M_PI * x) / (M_PI * x); }
+// Eq. 4: g[k] = sinc((k-c)/f) sinc((k-c)/c), c = f*half_len, k = 0..2c
+static std::vector<double> eq4_kernel(int f, int half_len) {
+  int c = f * half_len;
+  std::vector<double> g(2 * c + 1);
+  for (int k = 0; k <= 2 * c; ++k) g[k] = sinc_pi((double)(k - c) / f) * sinc_pi((double)(k - c) / c);
+  return g;
+}
+
+template <typename T>
+static cudaError_t dev_alloc(lloid_stream *s, T **p, size_t count, bool is_state = false) {
+  void *q = nullptr;
+  size_t bytes = std::max<size_t>(count * sizeof(T), 16);
+  cudaError_t e = cudaMalloc(&q, bytes);
+  if (e != cudaSuccess) return e;
+  e = cudaMemset(q, 0, bytes);
+  s->allocs.push_back(q);
+  if (is_state) s->state.push_back({q, bytes});
+  *p = (T *)q;
+  return e;
+}
+template <typename T>
+static cudaError_t dev_upload(lloid_stream *s, T **p, const std::vector<T> &h) {
+  cudaError_t e = dev_alloc(s, p, h.size());
+  if (e != cudaSuccess || h.empty()) return e;
+  return cudaMemcpy(*p, h.data(), h.size() * sizeof(T), cudaMemcpyHostToDevice);
+}
+
+extern "C" void lloid_stream_destroy(lloid_stream *s) {
+  if (!s) return;
+  if (s->tc) tc_plan_destroy(s->tc);
+  for (void *p : s->allocs) cudaFree(p);
+  delete s;
+}
+
+#define CK(expr)                                                                                   \
+  do {                                                                                             \
+    cudaError_t e_ = (expr);                                                                       \
+    if (e_ != cudaSuccess) {                                                                       \
+      set_error("stream_create: %s: %s", #expr, cudaGetErrorString(e_));                           \
+      lloid_stream_destroy(s);                                                                     \
+      return (e_ == cudaErrorMemoryAllocation) ? LLOID_ENOMEM : LLOID_ECUDA;                       \
+    }                                                                                              \
+  } while (0)
+
+extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *banks, int32_t n_banks,
+                                   int32_t n_det, int32_t B, void *cuda_stream) {
+  if (!out) { set_error("stream_create: out is NULL"); return LLOID_EINVAL; }
+  *out = nullptr;
+  if (!banks || n_banks < 1 || n_det < 1 || B < 1) { set_error("stream_create: need banks, n_banks, n_detectors, buffer_len >= 1"); return LLOID_EINVAL; }
+  int Dmax = 1;
+  for (int b = 0; b < n_banks; ++b) {
+    if (!banks[b]) { set_error("stream_create: bank %d is NULL", b); return LLOID_EINVAL; }
+    if (banks[b]->f0 != banks[0]->f0 || banks[b]->opt.precision != banks[0]->opt.precision ||
+        banks[b]->opt.n_down != banks[0]->opt.n_down) {
+      set_error("stream_create: bank %d differs from bank 0 in strain rate, precision or n_down", b); return LLOID_EINVAL;
+    }
+    for (const SliceInfo &si : banks[b]->slices) Dmax = std::max(Dmax, si.D);
+  }
+  if (B % Dmax != 0) { set_error("stream_create: buffer_len %d is not a multiple of the largest decimation factor %d", B, Dmax); return LLOID_EINVAL; }
+  lloid_stream *s = new (std::nothrow) lloid_stream();
+  if (!s) { set_error("stream_create: out of host memory"); return LLOID_ENOMEM; }
+  s->banks.assign(banks, banks + n_banks);
+  s->n_det = n_det; s->B = B; s->f0 = banks[0]->f0; s->precision = banks[0]->opt.precision;
+  s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold;
+  s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr;
+  s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
+  const int planes = std::max(1, s->up_planes);
+  s->up_chunk = std::min(B, 256);
+  memset(s->work, 0, sizeof(s->work));
+  int dev = 0; cudaDeviceProp prop;
+  CK(cudaGetDevice(&dev));
+  CK(cudaGetDeviceProperties(&prop, dev));
+  if (prop.major != 10) { set_error("stream_create: device %s is sm_%d%d, this library is sm_100a only", prop.name, prop.major, prop.minor); lloid_stream_destroy(s); return LLOID_ECUDA; }
+  CK(dev_alloc(s, &s->n0_dev, 1, true));
+
+  // ---- rates and their rings
+  std::map<int, long long> span;                       // D -> max(delay + N) over slices at that rate
+  for (const lloid_bank *bk : s->banks)
+    for (const SliceInfo &si : bk->slices) span[si.D] = std::max(span[si.D], si.delay + si.N);
+  if ((int)span.size() > LLOID_MAX_RATES) { set_error("stream_create: more than %d distinct rates", LLOID_MAX_RATES); lloid_stream_destroy(s); return LLOID_EINVAL; }
+  std::map<int, int> rate_index;
+  DecimParams &dp = s->dec;
+  memset(&dp, 0, sizeof(dp));
+  dp.n_det = n_det; dp.B = B; dp.copy_blocks = std::max(1, std::min(8, B / 256));
+  int out_begin = 0;
+  for (auto &kv : span) {
+    int D = kv.first, ri = dp.n_rates++;
+    rate_index[D] = ri;
+    RateDev &r = dp.r[ri];
+    r.D = D; r.lag = (D == 1) ? 0 : s->n_down; r.c = s->n_down * D; r.n_out = B / D;
+    long long need = B / D + kv.second + 256;
+    if (D == 1) need = std::max<long long>(need, B + 2LL * s->n_down * Dmax + 256);
+    r.rlen = (int)need;
+    CK(dev_alloc(s, &r.ring2, (size_t)n_det * 2 * r.rlen, true));
+    r.taps = nullptr; r.out_begin = 0;
+    if (D > 1) {
+      std::vector<double> g = eq4_kernel(D, s->n_down);
+      double sum = 0; for (double v : g) sum += v;
+      std::vector<float> t(g.size());
+      for (size_t k = 0; k < g.size(); ++k) t[k] = (float)(std::sqrt((double)D) * g[k] / sum);
+      float *td; CK(dev_upload(s, &td, t)); r.taps = td;
+      r.out_begin = out_begin; out_begin += r.n_out;
+    }
+  }
+  dp.total_out = out_begin;
+
+  // ---- geometry classes: slices with equal (D, N, delay, H) share one Hankel operand; stack their U rows
+  typedef std::tuple<int, int, long long, int> Key;
+  std::map<Key, int> class_of;
+  std::vector<std::vector<std::pair<int, int>>> members;     // class -> (bank, slice)
+  std::vector<std::vector<int>> row_off(n_banks);
+  for (int b = 0; b < n_banks; ++b) {
+    const lloid_bank *bk = s->banks[b];
+    row_off[b].resize(bk->S);
+    for (int i = 0; i < bk->S; ++i) {
+      const SliceInfo &si = bk->slices[i];
+      Key key(si.D, si.N, si.delay, bk->groups[si.group].H);
+      auto it = class_of.find(key);
+      int c;
+      if (it == class_of.end()) {
+        c = (int)s->classes.size(); class_of[key] = c; members.emplace_back();
+        CorrClass cc; memset(&cc, 0, sizeof(cc));
+        const RateDev &r = dp.r[rate_index[si.D]];
+        cc.ring2 = r.ring2; cc.ring_det_stride = 2LL * r.rlen; cc.rlen = r.rlen; cc.lag = r.lag; cc.D = si.D;
+        cc.N = si.N; cc.Npad = (si.N + 63) / 64 * 64; cc.H = bk->groups[si.group].H; cc.delay = si.delay;
+        cc.ncols = B / si.D; cc.ylen = B / si.D + 32; cc.u_scale_inv = 1.f;
+        s->classes.push_back(cc);
+      } else c = it->second;
+      row_off[b][i] = s->classes[c].Lstack;
+      s->classes[c].Lstack += si.L;
+      members[c].push_back({b, i});
+    }
+  }
+  std::vector<CorrTile> tiles;
+  for (size_t c = 0; c < s->classes.size(); ++c) {
+    CorrClass &cc = s->classes[c];
+    cc.Lpad = (cc.Lstack + 127) / 128 * 128;
+    std::vector<float> U((size_t)cc.Lpad * cc.Npad, 0.f);
+    int row = 0;
+    for (auto &m : members[c]) {
+      const SliceInfo &si = s->banks[m.first]->slices[m.second];
+      for (int l = 0; l < si.L; ++l, ++row) memcpy(&U[(size_t)row * cc.Npad], &si.U[(size_t)l * si.N], sizeof(float) * si.N);
+    }
+    if (s->precision == LLOID_PREC_FP32_FFMA) {
+      float *p; CK(dev_upload(s, &p, U)); cc.U32 = p;
+    } else {
+      // fp16 operand planes; orthonormal rows have entries ~1/sqrt(N): scale by 2^ceil(log2 sqrt(N)) first
+      int ex = (int)std::ceil(0.5 * std::log2((double)cc.N)) + 2;
+      float sc = std::ldexp(1.f, ex);
+      cc.u_scale_inv = 1.f / sc;
+      std::vector<__half> U16(U.size() * planes);
+      for (size_t i = 0; i < U.size(); ++i) {
+        float v = U[i] * sc; __half h = __float2half_rn(v);
+        U16[i] = h;
+        if (planes == 2) U16[U.size() + i] = __float2half_rn(v - __half2float(h));
+      }
+      __half *p; CK(dev_upload(s, &p, U16)); cc.U16 = p;
+    }
+    CK(dev_alloc(s, &cc.yring, (size_t)n_det * cc.ylen * cc.Lpad, true));
+    cc.ydet_stride = (long long)cc.ylen * cc.Lpad;
+    for (int r0 = 0; r0 < cc.Lstack; r0 += 64)
+      for (int c0 = 0; c0 < cc.ncols; c0 += 64) tiles.push_back({(int)c, r0, c0});
+    s->work[0] += 2.0 * cc.Lpad * cc.Npad * cc.ncols * n_det;               // executed (padded) flop, one pass
+    s->work[2] += 2.0 * cc.Lstack * (double)cc.N * cc.ncols * n_det;
+    s->work[4] += (double)cc.Lpad * cc.Npad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
+    s->work[5] += 2.0 * 4.0 * cc.Lstack * cc.ncols * n_det;
+  }
+  CK(dev_upload(s, &s->classes_dev, s->classes));
+  s->n_tiles = (int)tiles.size();
+  CK(dev_upload(s, &s->tiles_dev, tiles));
+
+  // ---- upsampler taps (Eq. 4 with c = 8 f, not normalised) for f = 2 .. 2^11
+  {
+    std::vector<float> taps; std::vector<int> off(LLOID_MAX_GROUPS + 1, 0);
+    for (int lf = 1; lf <= LLOID_MAX_GROUPS; ++lf) {
+      if ((1 << lf) > Dmax) { off[lf] = 0; continue; }
+      off[lf] = (int)taps.size();
+      std::vector<double> g = eq4_kernel(1 << lf, LLOID_NUP);
+      for (double v : g) taps.push_back((float)v);
+    }
+    if (taps.empty()) taps.push_back(0.f);
+    CK(dev_upload(s, &s->uptaps_dev, taps));
+    CK(dev_upload(s, &s->uptap_off_dev, off));
+  }
+
+  // ---- per-bank Yup buffers, upsample items, reconstruction descriptors
+  std::vector<UpItem> items;
+  s->Mtot = 0; s->max_mtiles = 0;
+  for (int b = 0; b < n_banks; ++b) {
+    const lloid_bank *bk = s->banks[b];
+    ReconBank rb; memset(&rb, 0, sizeof(rb));
+    size_t plane_elems = (size_t)n_det * B * bk->Kpad;
+    void *yup = nullptr;
+    if (s->up_planes == 0) { float *p; CK(dev_alloc(s, &p, plane_elems)); yup = p; }
+    else { __half *p; CK(dev_alloc(s, &p, plane_elems * planes)); yup = p; }
+    rb.R32 = bk->dR32; rb.R16 = bk->dR16;
+    rb.r_part_stride = (long long)bk->Mpad * bk->Kpad; rb.r_plane_stride = 2 * rb.r_part_stride;
+    rb.yup = yup; rb.yup_det_stride = (long long)B * bk->Kpad; rb.yup_plane_stride = (long long)plane_elems;
+    rb.M = bk->M; rb.Mpad = bk->Mpad; rb.Kpad = bk->Kpad; rb.tmpl_off = s->Mtot;
+    rb.inv_scale = 1.f / bk->r_scale; rb.inv_scale2 = rb.inv_scale * rb.inv_scale;
+    s->rbanks.push_back(rb);
+    s->Mtot += bk->M;
+    s->max_mtiles = std::max(s->max_mtiles, (bk->M + 63) / 64);
+    double rate_sum = 0, up_out = 0;
+    for (int g = 0; g < bk->G; ++g) { if (g > 0) up_out += bk->groups[g - 1].rate; }
+    for (int i = 0; i < bk->S; ++i) {
+      const SliceInfo &si = bk->slices[i];
+      const CorrClass &cc = s->classes[class_of[Key(si.D, si.N, si.delay, bk->groups[si.group].H)]];
+      for (int l0 = 0; l0 < si.L; l0 += 32) {
+        UpItem it; memset(&it, 0, sizeof(it));
+        it.yring = cc.yring; it.ydet_stride = cc.ydet_stride; it.ylen = cc.ylen; it.ypitch = cc.Lpad;
+        it.row0 = row_off[b][i] + l0; it.nl = std::min(32, si.L - l0); it.kcol = si.koff + l0; it.g = si.group; it.D = si.D;
+        for (int h = 1; h <= si.group; ++h) it.log2f[h] = (int)std::lround(std::log2((double)bk->groups[h].f));
+        it.yup = yup; it.yup_det_stride = rb.yup_det_stride; it.yup_plane_stride = rb.yup_plane_stride; it.kpitch = bk->Kpad;
+        items.push_back(it);
+      }
+      rate_sum += (double)si.L * si.rate;
+    }
+    double secs = (double)B / s->f0;
+    s->work[1] += 2.0 * 2 * bk->Mpad * (double)bk->Kpad * B * n_det;
+    s->work[3] += (2.0 * 2 * bk->M * rate_sum + 16.0 * 2 * bk->M * up_out) * secs * n_det;
+    s->work[4] += 2.0 * bk->Mpad * bk->Kpad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
+    s->work[5] += 2.0 * plane_elems * (s->up_planes == 0 ? 4 : 2 * planes);
+  }
+  s->n_items = (int)items.size();
+  CK(dev_upload(s, &s->items_dev, items));
+  CK(dev_upload(s, &s->rbanks_dev, s->rbanks));
+  s->n_tt = (s->precision == LLOID_PREC_FP32_FFMA) ? (B + 63) / 64 : tc_time_splits(B);
+  CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
+  CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
+  CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
+  if (s->precision != LLOID_PREC_FP32_FFMA) {
+    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes);
+    if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
+    s->work[0] *= (planes == 2 ? 3 : 1);
+    s->work[1] *= (planes == 2 ? 3 : 1);
+  }
+  CK(cudaDeviceSynchronize());
+  *out = s;
+  return LLOID_OK;
+}
+#undef CK
+
+extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_peak *peaks, float *snr_debug,
+                                 int32_t debug_bank) {
+  if (!s || !strain || !peaks) { set_error("stream_push: stream, strain and peaks must be non-NULL"); return LLOID_EINVAL; }
+  if (snr_debug && (debug_bank < 0 || debug_bank >= (int)s->banks.size())) { set_error("stream_push: debug_bank %d out of range", debug_bank); return LLOID_ESTATE; }
+  cudaError_t e = launch_decimate(s->dec, strain, s->n0_dev, s->st);
+  if (e == cudaSuccess) {
+    if (s->tc) e = tc_launch_corr(s->tc, s->n0_dev, s->st);
+    else e = launch_corr_ffma(s->classes_dev, s->tiles_dev, s->n_tiles, s->n_det, s->n0_dev, s->st);
+  }
+  if (e == cudaSuccess)
+    e = launch_upsample(s->items_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
+                        s->n0_dev, s->up_planes, s->st);
+  if (e == cudaSuccess) {
+    if (s->tc) e = tc_launch_recon(s->tc, s->partial_dev, s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
+    else e = launch_recon_ffma(s->rbanks_dev, (int)s->banks.size(), s->max_mtiles, s->n_det, s->B, s->partial_dev,
+                               s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
+  }
+  if (e == cudaSuccess)
+    e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->st);
+  if (e != cudaSuccess) { set_error("stream_push: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  s->n0_host += s->B;
+  return LLOID_OK;
+}
+
+extern "C" int lloid_stream_push_host(lloid_stream *s, const float *strain_host, lloid_peak *peaks_host) {
+  if (!s || !strain_host || !peaks_host) { set_error("stream_push_host: NULL argument"); return LLOID_EINVAL; }
+  cudaError_t e = cudaMemcpyAsync(s->strain_dev, strain_host, sizeof(float) * s->n_det * s->B, cudaMemcpyHostToDevice, s->st);
+  if (e != cudaSuccess) { set_error("stream_push_host: H2D copy: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  int rc = lloid_stream_push(s, s->strain_dev, s->peaks_dev, nullptr, -1);
+  if (rc != LLOID_OK) return rc;
+  e = cudaMemcpyAsync(peaks_host, s->peaks_dev, sizeof(lloid_peak) * s->n_det * s->Mtot, cudaMemcpyDeviceToHost, s->st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->st);
+  if (e != cudaSuccess) { set_error("stream_push_host: D2H copy / sync: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  return LLOID_OK;
+}
+
+extern "C" int lloid_state_reset(lloid_stream *s) {
+  if (!s) { set_error("state_reset: stream is NULL"); return LLOID_EINVAL; }
+  for (auto &p : s->state) {
+    cudaError_t e = cudaMemsetAsync(p.first, 0, p.second, s->st);
+    if (e != cudaSuccess) { set_error("state_reset: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  }
+  s->n0_host = 0;
+  return LLOID_OK;
+}
+
+extern "C" int64_t lloid_stream_samples_pushed(const lloid_stream *s) { return s ? s->n0_host : -1; }
+extern "C" int32_t lloid_stream_total_templates(const lloid_stream *s) { return s ? s->Mtot : -1; }
+extern "C" int32_t lloid_stream_launches_per_push(const lloid_stream *s) { return s ? 5 : -1; }
+extern "C" int lloid_stream_work_per_push(const lloid_stream *s, double out[6]) {
+  if (!s || !out) { set_error("work_per_push: NULL argument"); return LLOID_EINVAL; }
+  for (int i = 0; i < 6; ++i) out[i] = s->work[i];
+  return LLOID_OK;
+}

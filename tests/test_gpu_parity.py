@@ -1,0 +1,125 @@
+"""GPU parity: the CUDA path (through the C ABI) against the float64 oracle, element by element (-m gpu).
+
+Tolerances (BASELINE.json north_star): max_k |z_gpu - z_oracle| <= tol * rms(|z_oracle|),
+tol = 1e-4 for LLOID_PREC_FP32_FFMA and 2e-3 for the tcgen05 modes; peak template/sample indices bit-exact for
+injected templates at SNR >= 8; elsewhere a GPU peak is accepted when the oracle's |z| at the GPU's sample is
+within tolerance of the oracle's maximum (several samples can be the maximum up to rounding).
+"""
+import numpy as np
+import pytest
+
+pytestmark = pytest.mark.gpu
+
+TOL = {0: 1e-4, 1: 2e-3, 2: 2e-3}
+
+
+def _torch_cuda():
+    torch = pytest.importorskip("torch")
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    return torch
+
+
+def run_gpu(banks, strain, B, precision, want_bank=0, n_push=None):
+    """Push strain [n_det][n] in buffers of B; return (rho [n_det][2M][n_push*B], peaks [n_push][n_det][Mtot])."""
+    import paper_2511_04730_b200 as lib
+    st = lib.LloidStream(banks, strain.shape[0], B, precision=precision)
+    n_push = strain.shape[1] // B if n_push is None else n_push
+    rho, peaks = [], []
+    for p in range(n_push):
+        pk, snr = st.push(strain[:, p * B:(p + 1) * B], want_snr_bank=want_bank)
+        rho.append(snr)
+        peaks.append(pk.copy())
+    st.close()
+    return np.concatenate(rho, axis=2), np.stack(peaks)
+
+
+def check_snr(rho_gpu, rho_ref, tol):
+    z_ref = rho_ref[0::2] + 1j * rho_ref[1::2]
+    z_gpu = rho_gpu[0::2] + 1j * rho_gpu[1::2]
+    rms = np.sqrt(np.mean(np.abs(z_ref) ** 2))
+    err = np.abs(z_gpu - z_ref)
+    return err.max() / rms, np.sqrt(np.mean(err ** 2)) / rms
+
+
+def check_peaks(pk, rho_ref, B, tol_abs, must_match=()):
+    """pk: [n_push][M] structured GPU peaks of one bank+detector; rho_ref [2M][n_push*B] float64."""
+    from oracle import find_peaks
+    snr, idx, ph = find_peaks(rho_ref, B)
+    n_push, M = snr.shape
+    for (p, j) in must_match:
+        assert pk["sample"][p, j] == idx[p, j], (p, j, pk["sample"][p, j], idx[p, j])
+    z = rho_ref[0::2] + 1j * rho_ref[1::2]
+    for p in range(n_push):
+        k = pk["sample"][p].astype(np.int64)
+        assert (k >= 0).all() and (k < B).all()
+        at = np.abs(z[np.arange(M), p * B + k])
+        assert (snr[p] - at <= tol_abs).all(), f"push {p}: GPU peak sample is not a maximum of the oracle SNR"
+        assert np.abs(pk["snr"][p] - at).max() <= tol_abs
+        dphi = np.angle(np.exp(1j * (pk["phase"][p] - np.angle(z[np.arange(M), p * B + k]))))
+        assert np.abs(dphi * at).max() <= 2 * tol_abs
+    return float(np.mean(pk["sample"] == idx))
+
+
+@pytest.mark.parametrize("precision", [0])
+def test_config1_full_snr_and_peaks(cfg1, precision):
+    """BASELINE.json configs[0]: 64 templates, 2 slices (2048 Hz, 512 Hz, one x4 stage), 16 s, 2 injections."""
+    _torch_cuda()
+    from oracle import lloid_snr
+    c, bank = cfg1["cfg"], cfg1["bank32"]
+    strain = cfg1["strain"]
+    B = c.buffer_len
+    rho_gpu, peaks = run_gpu([bank], strain, B, precision)
+    rho_ref = lloid_snr(bank, strain[0])
+    emax, erms = check_snr(rho_gpu[0], rho_ref, TOL[precision])
+    print(f"config1 precision={precision}: max err {emax:.3e} rms err {erms:.3e} (of SNR rms)")
+    assert emax <= TOL[precision]
+    rms = np.sqrt(np.mean(rho_ref[0::2] ** 2 + rho_ref[1::2] ** 2))
+    must = [(inj.k0 // B, inj.template) for inj in cfg1["inj"]]
+    frac = check_peaks(peaks[:, 0, :], rho_ref, B, TOL[precision] * rms * 2, must)
+    print(f"  peak sample agreement {frac:.4f}")
+    for inj in cfg1["inj"]:
+        p, j = inj.k0 // B, inj.template
+        assert peaks["sample"][p, 0, j] == inj.k0 % B          # recovered at the injected sample
+        assert abs(peaks["snr"][p, 0, j] - inj.amp) < 0.08 * inj.amp + 3.0
+
+
+@pytest.mark.parametrize("precision", [0])
+def test_chunk_invariance_and_reset(cfg1, precision):
+    """Streaming in 512-sample buffers equals streaming in 2048-sample buffers; reset restores sample 0."""
+    _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    bank, strain = cfg1["bank32"], cfg1["strain"][:, :4 * 2048]
+    a, _ = run_gpu([bank], strain, 2048, precision)
+    b, _ = run_gpu([bank], strain, 512, precision)
+    rms = np.sqrt(2.0)
+    assert np.abs(a - b).max() <= 2e-5 * rms
+    st = lib.LloidStream([bank], 1, 2048, precision=precision)
+    _, s1 = st.push(strain[:, :2048], want_snr_bank=0)
+    st.push(strain[:, 2048:4096])
+    st.reset()
+    _, s2 = st.push(strain[:, :2048], want_snr_bank=0)
+    assert np.array_equal(s1, s2)
+    st.close()
+
+
+@pytest.mark.parametrize("precision", [0])
+def test_multirate_bank_two_detectors(precision):
+    """A 5-rate chirp bank (2048..128 Hz, two slices at one rate) x 2 detectors, ragged M, against the oracle."""
+    _torch_cuda()
+    from oracle import lloid_snr
+    from workloads import bank_from_layout, make_strain
+    mc = np.linspace(1.2, 1.4, 37)            # M = 37: ragged template tile
+    f0 = 2048
+    lay = [(2048, 0, 1024), (1024, 1024, 3072), (512, 3072, 8192), (256, 8192, 16384), (256, 16384, 24576),
+           (128, 24576, 32768)]
+    bank = bank_from_layout(mc, 16.0, lay, f0=f0).as_f32()
+    strain = np.stack([make_strain(11, 8 * f0), make_strain(12, 8 * f0)])
+    B = 1024
+    rho_gpu, peaks = run_gpu([bank], strain, B, precision)
+    for det in range(2):
+        rho_ref = lloid_snr(bank, strain[det])
+        emax, erms = check_snr(rho_gpu[det], rho_ref, TOL[precision])
+        print(f"multirate det {det}: max err {emax:.3e} rms {erms:.3e}")
+        assert emax <= TOL[precision]
+        check_peaks(peaks[:, det, :], rho_ref, B, TOL[precision] * 2 * np.sqrt(2.0))
