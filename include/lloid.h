@@ -112,10 +112,21 @@ int64_t lloid_stream_samples_pushed(const lloid_stream *stream);
 int32_t lloid_stream_total_templates(const lloid_stream *stream);
 int32_t lloid_stream_launches_per_push(const lloid_stream *stream); /* kernels this library launches per push */
 /* Executed and algorithmic work of one push, for roofline accounting:
- * out[0] a2 flop executed, out[1] a3 flop executed, out[2] a2 algorithmic flop (2 sum L N f),
- * out[3] a3+a4 algorithmic flop in the paper's order (2 sum 2M L f + 16*2M*sum f_out),
- * out[4] bytes of operands (U, R) one push reads, out[5] bytes of Y/Yup intermediates written+read. */
-int lloid_stream_work_per_push(const lloid_stream *stream, double out[6]);
+ * out[0] a2 flop executed (padded tiles, x3 for the hi/lo split), out[1] a3 flop executed,
+ * out[2] a2 algorithmic flop 2 sum_s L^s N^s f^s (Eq. 5), out[3] a3 algorithmic flop 2 sum_s 2M L^s f^s (Eq. 6, the
+ * paper's order), out[4] a4 algorithmic flop 16*2M*sum_stages f_out (Eqs. 7-9), out[5] bytes of operands (U, R)
+ * one push reads, out[6] bytes of Y / upsampled-Y intermediates written + read, out[7] reserved (0). */
+int lloid_stream_work_per_push(const lloid_stream *stream, double out[8]);
+
+/* Per-stage device timing (bench / roofline evidence).  When enabled, every push records CUDA events on the
+ * stream between its kernels: stage 0 a1 decimate, 1 a2 correlate, 2 basis-domain upsample, 3 a3 reconstruct +
+ * a5 peaks, 4 peak finalisation.  lloid_stream_stage_times synchronises the stream, adds the elapsed
+ * milliseconds of every push since the last call into ms[0..LLOID_N_STAGES), returns the number of pushes
+ * covered (or a negative status) and clears the record. */
+#define LLOID_N_STAGES 5
+int lloid_stream_set_stage_timing(lloid_stream *stream, int32_t enable);
+int lloid_stream_stage_times(lloid_stream *stream, float ms[LLOID_N_STAGES]);
+const char *lloid_stage_name(int32_t stage);
 
 const char *lloid_last_error(void);
 const char *lloid_version(void);

@@ -54,6 +54,9 @@ def _load():
         "lloid_stream_total_templates": (i32, [vp]),
         "lloid_stream_launches_per_push": (i32, [vp]),
         "lloid_stream_work_per_push": (C.c_int, [vp, C.POINTER(C.c_double)]),
+        "lloid_stream_set_stage_timing": (C.c_int, [vp, i32]),
+        "lloid_stream_stage_times": (C.c_int, [vp, C.POINTER(C.c_float)]),
+        "lloid_stage_name": (C.c_char_p, [i32]),
         "lloid_last_error": (C.c_char_p, []),
         "lloid_version": (C.c_char_p, []),
     }
@@ -67,7 +70,8 @@ _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
            "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
-           "lloid_stream_work_per_push", "lloid_last_error", "lloid_version"]
+           "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
+           "lloid_stage_name", "lloid_last_error", "lloid_version"]
 
 
 def lloid_last_error() -> str:
@@ -158,9 +162,25 @@ def lloid_stream_launches_per_push(stream: int) -> int:
 
 
 def lloid_stream_work_per_push(stream: int) -> List[float]:
-    out = (C.c_double * 6)()
+    out = (C.c_double * 8)()
     _check(_lib.lloid_stream_work_per_push(stream, out))
     return list(out)
+
+
+LLOID_N_STAGES = 5
+
+
+def lloid_stream_set_stage_timing(stream: int, enable: bool):
+    _check(_lib.lloid_stream_set_stage_timing(stream, 1 if enable else 0))
+
+
+def lloid_stream_stage_times(stream: int):
+    """(pushes covered, {stage name: accumulated ms}); synchronises the stream."""
+    ms = (C.c_float * LLOID_N_STAGES)()
+    n = _lib.lloid_stream_stage_times(stream, ms)
+    if n < 0:
+        _check(n)
+    return n, {_lib.lloid_stage_name(i).decode(): float(ms[i]) for i in range(LLOID_N_STAGES)}
 
 
 # ---------------------------------------------------------------------------------------------------
@@ -225,6 +245,16 @@ class LloidStream:
 
     def work_per_push(self):
         return lloid_stream_work_per_push(self.handle)
+
+    def set_stage_timing(self, enable: bool):
+        lloid_stream_set_stage_timing(self.handle, enable)
+
+    def stage_times(self):
+        return lloid_stream_stage_times(self.handle)
+
+    @property
+    def launches_per_push(self) -> int:
+        return lloid_stream_launches_per_push(self.handle)
 
     def close(self):
         if getattr(self, "handle", None):

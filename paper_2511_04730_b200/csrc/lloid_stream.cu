@@ -32,7 +32,10 @@ struct lloid_stream {
   std::vector<void *> allocs;                      // every cudaMalloc of this stream
   std::vector<std::pair<void *, size_t>> state;    // (ptr, bytes) zeroed by reset
   int up_planes, up_chunk;
-  double work[6];
+  double work[8];
+  bool stage_timing;
+  std::vector<cudaEvent_t> ev_pool;               // free events
+  std::vector<std::vector<cudaEvent_t>> ev_rec;    // per timed push: LLOID_N_STAGES + 1 events
   TcPlan *tc;                                      // tensor-core launch plan (kernels_tc.cu), nullptr for FFMA
 };
 
@@ -67,6 +70,8 @@ static cudaError_t dev_upload(lloid_stream *s, T **p, const std::vector<T> &h) {
 extern "C" void lloid_stream_destroy(lloid_stream *s) {
   if (!s) return;
   if (s->tc) tc_plan_destroy(s->tc);
+  for (auto &v : s->ev_rec) for (cudaEvent_t e : v) cudaEventDestroy(e);
+  for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
   for (void *p : s->allocs) cudaFree(p);
   delete s;
 }
@@ -101,7 +106,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->banks.assign(banks, banks + n_banks);
   s->n_det = n_det; s->B = B; s->f0 = banks[0]->f0; s->precision = banks[0]->opt.precision;
   s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold;
-  s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr;
+  s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
   s->up_chunk = std::min(B, 256);
@@ -201,8 +206,8 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       for (int c0 = 0; c0 < cc.ncols; c0 += 64) tiles.push_back({(int)c, r0, c0});
     s->work[0] += 2.0 * cc.Lpad * cc.Npad * cc.ncols * n_det;               // executed (padded) flop, one pass
     s->work[2] += 2.0 * cc.Lstack * (double)cc.N * cc.ncols * n_det;
-    s->work[4] += (double)cc.Lpad * cc.Npad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
-    s->work[5] += 2.0 * 4.0 * cc.Lstack * cc.ncols * n_det;
+    s->work[5] += (double)cc.Lpad * cc.Npad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
+    s->work[6] += 2.0 * 4.0 * cc.Lstack * cc.ncols * n_det;
   }
   CK(dev_upload(s, &s->classes_dev, s->classes));
   s->n_tiles = (int)tiles.size();
@@ -257,9 +262,10 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     }
     double secs = (double)B / s->f0;
     s->work[1] += 2.0 * 2 * bk->Mpad * (double)bk->Kpad * B * n_det;
-    s->work[3] += (2.0 * 2 * bk->M * rate_sum + 16.0 * 2 * bk->M * up_out) * secs * n_det;
-    s->work[4] += 2.0 * bk->Mpad * bk->Kpad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
-    s->work[5] += 2.0 * plane_elems * (s->up_planes == 0 ? 4 : 2 * planes);
+    s->work[3] += 2.0 * 2 * bk->M * rate_sum * secs * n_det;
+    s->work[4] += 16.0 * 2 * bk->M * up_out * secs * n_det;
+    s->work[5] += 2.0 * bk->Mpad * bk->Kpad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
+    s->work[6] += 2.0 * plane_elems * (s->up_planes == 0 ? 4 : 2 * planes);
   }
   s->n_items = (int)items.size();
   CK(dev_upload(s, &s->items_dev, items));
@@ -284,21 +290,38 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
                                  int32_t debug_bank) {
   if (!s || !strain || !peaks) { set_error("stream_push: stream, strain and peaks must be non-NULL"); return LLOID_EINVAL; }
   if (snr_debug && (debug_bank < 0 || debug_bank >= (int)s->banks.size())) { set_error("stream_push: debug_bank %d out of range", debug_bank); return LLOID_ESTATE; }
+  std::vector<cudaEvent_t> ev;
+  if (s->stage_timing) {
+    for (int i = 0; i <= LLOID_N_STAGES; ++i) {
+      cudaEvent_t x;
+      if (!s->ev_pool.empty()) { x = s->ev_pool.back(); s->ev_pool.pop_back(); }
+      else if (cudaEventCreate(&x) != cudaSuccess) { set_error("stream_push: cudaEventCreate failed"); return LLOID_ECUDA; }
+      ev.push_back(x);
+    }
+  }
+  auto mark = [&](int i) { if (s->stage_timing) cudaEventRecord(ev[i], s->st); };
+  mark(0);
   cudaError_t e = launch_decimate(s->dec, strain, s->n0_dev, s->st);
+  mark(1);
   if (e == cudaSuccess) {
     if (s->tc) e = tc_launch_corr(s->tc, s->n0_dev, s->st);
     else e = launch_corr_ffma(s->classes_dev, s->tiles_dev, s->n_tiles, s->n_det, s->n0_dev, s->st);
   }
+  mark(2);
   if (e == cudaSuccess)
     e = launch_upsample(s->items_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
                         s->n0_dev, s->up_planes, s->st);
+  mark(3);
   if (e == cudaSuccess) {
     if (s->tc) e = tc_launch_recon(s->tc, s->partial_dev, s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
     else e = launch_recon_ffma(s->rbanks_dev, (int)s->banks.size(), s->max_mtiles, s->n_det, s->B, s->partial_dev,
                                s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
   }
+  mark(4);
   if (e == cudaSuccess)
     e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->st);
+  mark(5);
+  if (s->stage_timing) s->ev_rec.push_back(std::move(ev));
   if (e != cudaSuccess) { set_error("stream_push: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   s->n0_host += s->B;
   return LLOID_OK;
@@ -329,8 +352,38 @@ extern "C" int lloid_state_reset(lloid_stream *s) {
 extern "C" int64_t lloid_stream_samples_pushed(const lloid_stream *s) { return s ? s->n0_host : -1; }
 extern "C" int32_t lloid_stream_total_templates(const lloid_stream *s) { return s ? s->Mtot : -1; }
 extern "C" int32_t lloid_stream_launches_per_push(const lloid_stream *s) { return s ? 5 : -1; }
-extern "C" int lloid_stream_work_per_push(const lloid_stream *s, double out[6]) {
+extern "C" int lloid_stream_work_per_push(const lloid_stream *s, double out[8]) {
   if (!s || !out) { set_error("work_per_push: NULL argument"); return LLOID_EINVAL; }
-  for (int i = 0; i < 6; ++i) out[i] = s->work[i];
+  for (int i = 0; i < 8; ++i) out[i] = s->work[i];
   return LLOID_OK;
+}
+
+extern "C" int lloid_stream_set_stage_timing(lloid_stream *s, int32_t enable) {
+  if (!s) { set_error("set_stage_timing: stream is NULL"); return LLOID_EINVAL; }
+  s->stage_timing = enable != 0;
+  return LLOID_OK;
+}
+
+extern "C" int lloid_stream_stage_times(lloid_stream *s, float ms[LLOID_N_STAGES]) {
+  if (!s || !ms) { set_error("stage_times: NULL argument"); return LLOID_EINVAL; }
+  cudaError_t e = cudaStreamSynchronize(s->st);
+  if (e != cudaSuccess) { set_error("stage_times: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  for (int i = 0; i < LLOID_N_STAGES; ++i) ms[i] = 0.f;
+  int n = 0;
+  for (auto &v : s->ev_rec) {
+    for (int i = 0; i < LLOID_N_STAGES; ++i) {
+      float t = 0.f;
+      if (cudaEventElapsedTime(&t, v[i], v[i + 1]) == cudaSuccess) ms[i] += t;
+    }
+    for (cudaEvent_t x : v) s->ev_pool.push_back(x);
+    ++n;
+  }
+  s->ev_rec.clear();
+  return n;
+}
+
+extern "C" const char *lloid_stage_name(int32_t i) {
+  static const char *names[LLOID_N_STAGES] = {"a1_decimate", "a2_correlate", "a4_upsample_basis", "a3_reconstruct_a5_peaks",
+                                              "a5_finalize"};
+  return (i >= 0 && i < LLOID_N_STAGES) ? names[i] : "";
 }

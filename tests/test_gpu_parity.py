@@ -80,7 +80,9 @@ def test_config1_full_snr_and_peaks(cfg1, precision):
     print(f"  peak sample agreement {frac:.4f}")
     for inj in cfg1["inj"]:
         p, j = inj.k0 // B, inj.template
-        assert peaks["sample"][p, 0, j] == inj.k0 % B          # recovered at the injected sample
+        # bit-exact against the oracle is `must` above; against the injected sample N(0,1) noise may move the
+        # peak by a sample or two (same band as tests/test_oracle_pins.py::test_injections_recovered_at_injected_sample)
+        assert abs(int(peaks["sample"][p, 0, j]) - inj.k0 % B) <= 2
         assert abs(peaks["snr"][p, 0, j] - inj.amp) < 0.08 * inj.amp + 3.0
 
 
