@@ -10,7 +10,9 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-TOL = {0: 1e-4, 1: 2e-3, 2: 2e-3}
+# precision 1 (operands rounded once to fp16) is NOT a north-star mode: its error near loud injections exceeds 2e-3
+# (DESIGN.md section 4); it is gated at 1e-2 only to prove the kernels' single-plane path.
+TOL = {0: 1e-4, 1: 1e-2, 2: 2e-3}
 
 
 def _torch_cuda():
@@ -61,7 +63,7 @@ def check_peaks(pk, rho_ref, B, tol_abs, must_match=()):
     return float(np.mean(pk["sample"] == idx))
 
 
-@pytest.mark.parametrize("precision", [0])
+@pytest.mark.parametrize("precision", [0, 2, 1])
 def test_config1_full_snr_and_peaks(cfg1, precision):
     """BASELINE.json configs[0]: 64 templates, 2 slices (2048 Hz, 512 Hz, one x4 stage), 16 s, 2 injections."""
     _torch_cuda()
@@ -86,7 +88,7 @@ def test_config1_full_snr_and_peaks(cfg1, precision):
         assert abs(peaks["snr"][p, 0, j] - inj.amp) < 0.08 * inj.amp + 3.0
 
 
-@pytest.mark.parametrize("precision", [0])
+@pytest.mark.parametrize("precision", [0, 2, 1])
 def test_chunk_invariance_and_reset(cfg1, precision):
     """Streaming in 512-sample buffers equals streaming in 2048-sample buffers; reset restores sample 0."""
     _torch_cuda()
@@ -105,7 +107,7 @@ def test_chunk_invariance_and_reset(cfg1, precision):
     st.close()
 
 
-@pytest.mark.parametrize("precision", [0])
+@pytest.mark.parametrize("precision", [0, 2, 1])
 def test_multirate_bank_two_detectors(precision):
     """A 5-rate chirp bank (2048..128 Hz, two slices at one rate) x 2 detectors, ragged M, against the oracle."""
     _torch_cuda()
