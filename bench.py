@@ -58,6 +58,22 @@ def build_workload(cfg_no, n_banks_limit, seconds, rank=0):
     return c, banks, strain
 
 
+def max_over_ranks(t_local, device, world):
+    """Timed-region seconds of the slowest rank (all_reduce MAX over the job's process group)."""
+    if world <= 1:
+        return float(t_local)
+    import torch
+    import torch.distributed as dist
+    t = torch.tensor([t_local], device=device, dtype=torch.float64)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def whole_job_value(world, units_per_step_per_rank, steps, seconds):
+    """Aggregate throughput of `world` independent replicas (weak scaling, no data-path collective)."""
+    return world * units_per_step_per_rank * steps / seconds
+
+
 class ClockSampler:
     """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
     Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -205,10 +221,7 @@ def run_ours(args):
     wall = time.perf_counter() - wall0
     clocks = sampler.stop()
     ms = [a.elapsed_time(b) for a, b in zip(ev0, ev1)]
-    t_dev = torch.tensor([sum(ms) / 1e3], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t_dev, op=dist.ReduceOp.MAX)
-    t_dev = float(t_dev.item())
+    t_dev = max_over_ranks(sum(ms) / 1e3, dev, world)
 
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D strain + push + D2H peaks per step
     t_e2e = 0.0
@@ -219,10 +232,7 @@ def run_ours(args):
         t0 = time.perf_counter()
         st.push_host()
         t_e2e += time.perf_counter() - t0
-    t_e2e_t = torch.tensor([t_e2e], device=dev, dtype=torch.float64)
-    if world > 1:
-        dist.all_reduce(t_e2e_t, op=dist.ReduceOp.MAX)
-    t_e2e = float(t_e2e_t.item())
+    t_e2e = max_over_ranks(t_e2e, dev, world)
 
     # ---- per-stage device times (CUDA events recorded by the library on its stream) for the roofline
     st.set_stage_timing(True)
@@ -258,8 +268,8 @@ def measured_peaks():
 
 def assemble(args, c, banks, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks):
     peaks, peak_src = measured_peaks()
-    value = world * units_per_step * K / t_dev
-    e2e = world * units_per_step * K / t_e2e
+    value = whole_job_value(world, units_per_step, K, t_dev)
+    e2e = whole_job_value(world, units_per_step, K, t_e2e)
     per_stage = {k: v / max(n_cov, 1) for k, v in stage_ms.items()}            # ms per push
     dom = max(per_stage, key=per_stage.get)
     dom_s = per_stage[dom] / 1e3
