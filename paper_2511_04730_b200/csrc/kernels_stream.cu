@@ -9,8 +9,9 @@ namespace lloid {
 // K1: append the pushed strain to the f0 ring and decimate it to every lower rate.
 //   d_r[j] = sum_k taps[k] * d[j*D + c - k], taps = sqrt(D)*ghat (host, float64 -> fp32), zero phase.
 //   New outputs of a push: j in [n0/D - n_down, (n0+B)/D - n_down)  (needs c future f0 samples).
-//   One warp per output; lane t sums taps t, t+32, ... in a fixed order, then a shuffle tree: deterministic.
+//   DEC_PER_CTA outputs per CTA; thread t sums taps t, t+256, ... then a fixed-order reduction: deterministic.
 // ------------------------------------------------------------------------------------------------
+#define DEC_PER_CTA 8
 __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, const float *__restrict__ strain,
                                                        const long long *__restrict__ n0_ptr) {
   const long long n0 = *n0_ptr;
@@ -28,36 +29,55 @@ __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, cons
     }
     return;
   }
-  const int warp = ((blockIdx.x - P.copy_blocks) * blockDim.x + threadIdx.x) >> 5;
-  const int lane = threadIdx.x & 31;
-  if (warp >= P.total_out) return;
-  int ri = 1;
-  while (ri + 1 < P.n_rates && warp >= P.r[ri + 1].out_begin) ++ri;
-  const RateDev &r = P.r[ri];
-  const long long j = n0 / r.D - r.lag + (warp - r.out_begin);
-  const long long top = j * r.D + r.c;            // f0 index read by tap k = 0
-  float acc = 0.f;
-  const int ntap = 2 * r.c + 1;
-  for (int k = lane; k < ntap; k += 32) {
-    long long i = top - k;
-    float v;
-    if (i >= n0) v = sd[i - n0];
-    else if (i < 0) v = 0.f;
-    else v = ring0[(int)(i % r0.rlen)];
-    acc = fmaf(r.taps[k], v, acc);
-  }
+  // DEC_PER_CTA consecutive (flattened) outputs per CTA; the 256 threads split the taps of each output, partial
+  // sums are reduced in a fixed order (lane tree, then warps 0..7): deterministic.
+  __shared__ float part[DEC_PER_CTA][8];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int o0 = (blockIdx.x - P.copy_blocks) * DEC_PER_CTA;
+#pragma unroll 1
+  for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
+    const int o = o0 + oi;
+    if (o >= P.total_out) break;
+    int ri = 1;
+    while (ri + 1 < P.n_rates && o >= P.r[ri + 1].out_begin) ++ri;
+    const RateDev &r = P.r[ri];
+    const long long j = n0 / r.D - r.lag + (o - r.out_begin);
+    const long long top = j * r.D + r.c;            // f0 index read by tap k = 0
+    float acc = 0.f;
+    const int ntap = 2 * r.c + 1;
+    for (int k = threadIdx.x; k < ntap; k += 256) {
+      long long i = top - k;
+      float v;
+      if (i >= n0) v = sd[i - n0];
+      else if (i < 0) v = 0.f;
+      else v = ring0[(int)(i % r0.rlen)];
+      acc = fmaf(r.taps[k], v, acc);
+    }
 #pragma unroll
-  for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
-  if (lane == 0) {
-    int slot = (int)((j + r.lag) % r.rlen);
-    float *ring = r.ring2 + (size_t)det * 2 * r.rlen;
-    ring[slot] = acc;
-    ring[slot + r.rlen] = acc;
+    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
+    if (lane == 0) part[oi][warp] = acc;
+  }
+  __syncthreads();
+  if (threadIdx.x < DEC_PER_CTA) {
+    const int o = o0 + threadIdx.x;
+    if (o < P.total_out) {
+      int ri = 1;
+      while (ri + 1 < P.n_rates && o >= P.r[ri + 1].out_begin) ++ri;
+      const RateDev &r = P.r[ri];
+      const long long j = n0 / r.D - r.lag + (o - r.out_begin);
+      float acc = 0.f;
+#pragma unroll
+      for (int w = 0; w < 8; ++w) acc += part[threadIdx.x][w];
+      int slot = (int)((j + r.lag) % r.rlen);
+      float *ring = r.ring2 + (size_t)det * 2 * r.rlen;
+      ring[slot] = acc;
+      ring[slot + r.rlen] = acc;
+    }
   }
 }
 
 cudaError_t launch_decimate(const DecimParams &P, const float *strain, const long long *n0, cudaStream_t st) {
-  int dec_blocks = (P.total_out + 7) / 8;
+  int dec_blocks = (P.total_out + DEC_PER_CTA - 1) / DEC_PER_CTA;
   dim3 grid(P.copy_blocks + dec_blocks, P.n_det);
   decimate_kernel<<<grid, 256, 0, st>>>(P, strain, n0);
   return cudaGetLastError();
@@ -74,77 +94,132 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 // ------------------------------------------------------------------------------------------------
 #define UP_MAXW 168   // widest staged level: chunk/2 + 2*8 + ... <= 256/2 + 33
 template <int HALF_PLANES>
+__device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_stride, float v) {
+  if (HALF_PLANES == 0) {
+    reinterpret_cast<float *>(yup)[o] = v;
+  } else {
+    __half hi16 = __float2half_rn(v);
+    reinterpret_cast<__half *>(yup)[o] = hi16;
+    if (HALF_PLANES == 2) reinterpret_cast<__half *>(yup)[o + plane_stride] = __float2half_rn(v - __half2float(hi16));
+  }
+}
+
+template <int HALF_PLANES>
 __global__ void __launch_bounds__(256) upsample_kernel(const UpItem *__restrict__ items, int B, int chunk,
                                                        const float *__restrict__ uptaps,
                                                        const int *__restrict__ uptap_off,
                                                        const long long *__restrict__ n0_ptr) {
   __shared__ float buf[2][UP_MAXW][32];
-  const UpItem it = items[blockIdx.y];
+  __shared__ int s_r0[LLOID_MAX_GROUPS + 1], s_w[LLOID_MAX_GROUPS + 1], s_lf[LLOID_MAX_GROUPS + 1], s_slot0;
+  const UpItem *it = &items[blockIdx.y];
   const int det = blockIdx.z;
-  const long long n0 = *n0_ptr;
   const int ka = blockIdx.x * chunk;
   const int kb = min(ka + chunk, B);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-  const bool active = lane < it.nl;
-
-  long long lo[LLOID_MAX_GROUPS + 1], hi[LLOID_MAX_GROUPS + 1];
-  lo[0] = n0 + ka;
-  hi[0] = n0 + kb;
-  for (int h = 1; h <= it.g; ++h) {
-    lo[h] = (lo[h - 1] >> it.log2f[h]) - LLOID_NUP;          // arithmetic shift = floor division
-    hi[h] = ((hi[h - 1] - 1) >> it.log2f[h]) + LLOID_NUP + 1;
-  }
-  const float *yr = it.yring + (size_t)det * it.ydet_stride + it.row0 + lane;
-  const size_t out_row0 = (size_t)det * it.yup_det_stride + (size_t)it.kcol + lane;
-
-  auto store_out = [&](int k, float v) {   // k: sample within the buffer
-    size_t o = out_row0 + (size_t)k * it.kpitch;
-    if (HALF_PLANES == 0) {
-      reinterpret_cast<float *>(it.yup)[o] = v;
-    } else {
-      __half hi16 = __float2half_rn(v);
-      reinterpret_cast<__half *>(it.yup)[o] = hi16;
-      if (HALF_PLANES == 2)
-        reinterpret_cast<__half *>(it.yup)[o + it.yup_plane_stride] = __float2half_rn(v - __half2float(hi16));
+  const int G = it->g;
+  // Level h covers the absolute index range [lo_h, hi_h) at its rate (64-bit, thread 0 only); everything the
+  // loops below need is relative and fits 32 bits: width w_h, phase r0_h = lo_{h-1} mod f_h of the first output of
+  // stage h, and the Y-ring slot of column lo_G.  lo_h = floor(lo_{h-1} / f_h) - 8, hi_h = floor((hi_{h-1} - 1) / f_h) + 9.
+  if (threadIdx.x == 0) {
+    long long lo = *n0_ptr + ka, hi = *n0_ptr + kb;
+    s_w[0] = (int)(hi - lo);
+    for (int h = 1; h <= G; ++h) {
+      const int lf = it->log2f[h];
+      s_lf[h] = lf;
+      s_r0[h] = (int)(lo & ((1 << lf) - 1));
+      lo = (lo >> lf) - LLOID_NUP;                   // arithmetic shift = floor division
+      hi = ((hi - 1) >> lf) + LLOID_NUP + 1;
+      s_w[h] = (int)(hi - lo);
     }
-  };
+    s_slot0 = (int)((lo + 64) % it->ylen);
+  }
+  __syncthreads();
+  const bool active = lane < it->nl;
+  const int ylen = it->ylen, ypitch = it->ypitch, kpitch = it->kpitch;
+  const float *yr = it->yring + (size_t)det * it->ydet_stride + it->row0 + lane;
+  void *yup = it->yup;
+  const size_t plane_stride = (size_t)it->yup_plane_stride;
+  const size_t out0 = (size_t)det * it->yup_det_stride + (size_t)it->kcol + lane + (size_t)ka * kpitch;   // sample ka
 
-  // level g from the Y ring (columns never computed at stream start are the ring's zeros)
-  const int wg = (int)(hi[it.g] - lo[it.g]);
-  if (it.g == 0) {
+  // level G from the Y ring (columns never computed at stream start are the ring's zeros)
+  const int wg = s_w[G];
+  int slot = s_slot0 + warp;
+  if (slot >= ylen) slot -= ylen;
+  if (G == 0) {
     for (int c = warp; c < wg; c += nwarp) {
-      long long j = lo[0] + c;
-      int slot = (int)((j + 64) % it.ylen);
-      if (active) store_out(ka + c, yr[(size_t)slot * it.ypitch]);
+      if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, yr[(size_t)slot * ypitch]);
+      slot += nwarp; if (slot >= ylen) slot -= ylen;
     }
     return;
   }
   for (int c = warp; c < wg; c += nwarp) {
-    long long j = lo[it.g] + c;
-    int slot = (int)((j + 64) % it.ylen);
-    buf[0][c][lane] = active ? yr[(size_t)slot * it.ypitch] : 0.f;
+    buf[0][c][lane] = active ? yr[(size_t)slot * ypitch] : 0.f;
+    slot += nwarp; if (slot >= ylen) slot -= ylen;
   }
   __syncthreads();
   int cur = 0;
-  for (int h = it.g; h >= 1; --h) {
-    const int lf = it.log2f[h], f = 1 << lf;
+  for (int h = G; h >= 1; --h) {
+    const int lf = s_lf[h], f = 1 << lf, r0 = s_r0[h], wout = s_w[h - 1];
     const float *g = uptaps + uptap_off[lf];
-    const int wout = (int)(hi[h - 1] - lo[h - 1]);
-    for (int c = warp; c < wout; c += nwarp) {
-      long long i = lo[h - 1] + c;
-      long long q = i >> lf;
-      int ph = (int)(i & (f - 1));
-      int base = (int)(q - lo[h]);           // index of in[q]
-      float v;
-      if (ph == 0) {
-        v = buf[cur][base][lane];
-      } else {
-        v = 0.f;
+    // Output c (relative to lo_{h-1}) has input index qq = (r0 + c) >> lf relative to floor(lo_{h-1}/f) and phase
+    // (r0 + c) & (f-1); in[qq] sits at buffer index qq + 8.  Each warp takes a run of consecutive qq and slides a
+    // 16-sample register window over it (window slot (j + u) & 15 holds in[qq - 7 + j]): 1 shared load per 16 FMA.
+    const int nq = ((r0 + wout - 1) >> lf) + 1, per = (nq + nwarp - 1) / nwarp;
+    const int qa = warp * per, qb = min(qa + per, nq);
+    const float(*in)[32] = buf[cur];
+    float(*out)[32] = buf[cur ^ 1];
+    if (qa < qb) {
+      float W[16], T[16];
 #pragma unroll
-        for (int k = 0; k < 2 * LLOID_NUP; ++k) v = fmaf(buf[cur][base + LLOID_NUP - k][lane], g[k * f + ph], v);
+      for (int j = 0; j < 15; ++j) W[j] = in[qa + 1 + j][lane];
+      if (f == 2) {
+#pragma unroll
+        for (int k = 0; k < 16; ++k) T[k] = g[2 * k + 1];
       }
-      if (h == 1) { if (active) store_out(ka + c, v); }
-      else buf[cur ^ 1][c][lane] = v;
+      for (int q0 = qa; q0 < qb; q0 += 16) {
+#pragma unroll
+        for (int u = 0; u < 16; ++u) {
+          const int qq = q0 + u;
+          if (qq < qb) {
+            W[(u + 15) & 15] = in[qq + 16][lane];
+            const int c0 = (qq << lf) - r0;                 // output of phase 0
+            if (c0 >= 0 && c0 < wout) {                     // phase 0: the copy of Eq. 8 case 1
+              const float v = W[(u + 7) & 15];
+              if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c0 * kpitch, plane_stride, v); }
+              else out[c0][lane] = v;
+            }
+            if (f == 2) {
+              const int c = c0 + 1;
+              if (c >= 0 && c < wout) {
+                float v0 = 0.f, v1 = 0.f;
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) {           // in[qq + 8 - k] sits in window slot (15 - k + u) & 15
+                  v0 = fmaf(W[(15 - k + u) & 15], T[k], v0);
+                  v1 = fmaf(W[(14 - k + u) & 15], T[k + 1], v1);
+                }
+                const float v = v0 + v1;
+                if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v); }
+                else out[c][lane] = v;
+              }
+            } else {
+              for (int ph = 1; ph < f; ++ph) {
+                const int c = c0 + ph;
+                if (c >= 0 && c < wout) {
+                  float v0 = 0.f, v1 = 0.f;
+#pragma unroll
+                  for (int k = 0; k < 16; k += 2) {
+                    v0 = fmaf(W[(15 - k + u) & 15], g[k * f + ph], v0);
+                    v1 = fmaf(W[(14 - k + u) & 15], g[(k + 1) * f + ph], v1);
+                  }
+                  const float v = v0 + v1;
+                  if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v); }
+                  else out[c][lane] = v;
+                }
+              }
+            }
+          }
+        }
+      }
     }
     __syncthreads();
     cur ^= 1;
