@@ -1,6 +1,8 @@
 // a1 decimator (Eq. 4), the basis-domain polyphase upsampler (Eqs. 7-9)
 // and the peak finalisation.  FP32 CUDA-core kernels shared by every precision mode:
 // they are latency/HBM-bound stages, not contractions.
+#include <cmath>
+
 #include "lloid_internal.h"
 
 namespace lloid {
@@ -92,6 +94,8 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   sum_{k=0}^{15} in[floor(i/f) + 8 - k] * g_f[k f + (i mod f)]   (Eq. 7-8, zero-phase form).
 //   CTA = (time chunk of `chunk` f0 samples, item = 32 basis rows of one slice, detector).  lane = basis row.
 // ------------------------------------------------------------------------------------------------
+#define UP_RUN 8
+struct UpTaps2 { float t[16]; };   // g_2[2k+1], k = 0..15: the 16 non-zero taps of the x2 interpolation phase (Eq. 7)
 #define UP_MAXW 168   // widest staged level: chunk/2 + 2*8 + ... <= 256/2 + 33
 template <int HALF_PLANES>
 __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_stride, float v) {
@@ -105,10 +109,10 @@ __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_strid
 }
 
 template <int HALF_PLANES>
-__global__ void __launch_bounds__(256) upsample_kernel(const UpItem *__restrict__ items, int B, int chunk,
-                                                       const float *__restrict__ uptaps,
-                                                       const int *__restrict__ uptap_off,
-                                                       const long long *__restrict__ n0_ptr) {
+__global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restrict__ items, int B, int chunk,
+                                                          const float *__restrict__ uptaps,
+                                                          const int *__restrict__ uptap_off,
+                                                          const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
   __shared__ float buf[2][UP_MAXW][32];
   __shared__ int s_r0[LLOID_MAX_GROUPS + 1], s_w[LLOID_MAX_GROUPS + 1], s_lf[LLOID_MAX_GROUPS + 1], s_slot0;
   const UpItem *it = &items[blockIdx.y];
@@ -146,75 +150,100 @@ __global__ void __launch_bounds__(256) upsample_kernel(const UpItem *__restrict_
   int slot = s_slot0 + warp;
   if (slot >= ylen) slot -= ylen;
   if (G == 0) {
-    for (int c = warp; c < wg; c += nwarp) {
-      if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, yr[(size_t)slot * ypitch]);
-      slot += nwarp; if (slot >= ylen) slot -= ylen;
+    for (int c = warp; c < wg; c += 4 * nwarp) {
+      float v[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        v[i] = (active && c + i * nwarp < wg) ? yr[(size_t)slot * ypitch] : 0.f;
+        slot += nwarp; if (slot >= ylen) slot -= ylen;
+      }
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+        if (active && c + i * nwarp < wg) up_store<HALF_PLANES>(yup, out0 + (size_t)(c + i * nwarp) * kpitch, plane_stride, v[i]);
     }
     return;
   }
-  for (int c = warp; c < wg; c += nwarp) {
-    buf[0][c][lane] = active ? yr[(size_t)slot * ypitch] : 0.f;
-    slot += nwarp; if (slot >= ylen) slot -= ylen;
+  for (int c = warp; c < wg; c += 4 * nwarp) {            // 4 independent loads in flight per warp
+    float v[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      v[i] = (active && c + i * nwarp < wg) ? yr[(size_t)slot * ypitch] : 0.f;
+      slot += nwarp; if (slot >= ylen) slot -= ylen;
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i) if (c + i * nwarp < wg) buf[0][c + i * nwarp][lane] = v[i];
   }
   __syncthreads();
   int cur = 0;
   for (int h = G; h >= 1; --h) {
     const int lf = s_lf[h], f = 1 << lf, r0 = s_r0[h], wout = s_w[h - 1];
-    const float *g = uptaps + uptap_off[lf];
     // Output c (relative to lo_{h-1}) has input index qq = (r0 + c) >> lf relative to floor(lo_{h-1}/f) and phase
-    // (r0 + c) & (f-1); in[qq] sits at buffer index qq + 8.  Each warp takes a run of consecutive qq and slides a
-    // 16-sample register window over it (window slot (j + u) & 15 holds in[qq - 7 + j]): 1 shared load per 16 FMA.
+    // (r0 + c) & (f-1); in[qq] sits at buffer index qq + 8.  Each warp takes a run of consecutive qq, UP_RUN at a time,
+    // with the run's inputs held in registers: ~3 shared loads per 16 FMA, no per-tap index arithmetic.
     const int nq = ((r0 + wout - 1) >> lf) + 1, per = (nq + nwarp - 1) / nwarp;
     const int qa = warp * per, qb = min(qa + per, nq);
     const float(*in)[32] = buf[cur];
     float(*out)[32] = buf[cur ^ 1];
-    if (qa < qb) {
-      float W[16], T[16];
+    for (int q0 = qa; q0 < qb; q0 += UP_RUN) {
+      // the run's inputs in[q0 - 7 .. q0 + UP_RUN + 7] (buffer index q0 + 1 + j) held in registers:
+      // in[qq + 8 - k] = X[u + 15 - k] for qq = q0 + u
+      const int nrun = min(UP_RUN, qb - q0);
+      float X[UP_RUN + 15];
 #pragma unroll
-      for (int j = 0; j < 15; ++j) W[j] = in[qa + 1 + j][lane];
+      for (int j = 0; j < UP_RUN + 15; ++j) X[j] = (j < nrun + 15) ? in[q0 + 1 + j][lane] : 0.f;
+      const int cbase = (q0 << lf) - r0;                    // output index of (u = 0, phase 0)
       if (f == 2) {
+        // taps g_2[2k+1] come from the kernel parameter (constant bank): FFMA with a constant operand
+        float odd[UP_RUN];
 #pragma unroll
-        for (int k = 0; k < 16; ++k) T[k] = g[2 * k + 1];
-      }
-      for (int q0 = qa; q0 < qb; q0 += 16) {
+        for (int u = 0; u < UP_RUN; ++u) {
+          float v0 = 0.f, v1 = 0.f;
 #pragma unroll
-        for (int u = 0; u < 16; ++u) {
-          const int qq = q0 + u;
-          if (qq < qb) {
-            W[(u + 15) & 15] = in[qq + 16][lane];
-            const int c0 = (qq << lf) - r0;                 // output of phase 0
-            if (c0 >= 0 && c0 < wout) {                     // phase 0: the copy of Eq. 8 case 1
-              const float v = W[(u + 7) & 15];
-              if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c0 * kpitch, plane_stride, v); }
-              else out[c0][lane] = v;
+          for (int k = 0; k < 16; k += 2) {
+            v0 = fmaf(X[u + 15 - k], taps2.t[k], v0);
+            v1 = fmaf(X[u + 14 - k], taps2.t[k + 1], v1);
+          }
+          odd[u] = v0 + v1;
+        }
+        if (h == 1) {
+          size_t o = out0 + (size_t)max(cbase, 0) * kpitch;
+#pragma unroll
+          for (int u = 0; u < UP_RUN; ++u) {
+            const int c0 = cbase + 2 * u;
+            if (u < nrun && active) {
+              if (c0 >= 0 && c0 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]); o += kpitch; }
+              if (c0 + 1 >= 0 && c0 + 1 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, odd[u]); o += kpitch; }
             }
-            if (f == 2) {
-              const int c = c0 + 1;
-              if (c >= 0 && c < wout) {
-                float v0 = 0.f, v1 = 0.f;
+          }
+        } else {
 #pragma unroll
-                for (int k = 0; k < 16; k += 2) {           // in[qq + 8 - k] sits in window slot (15 - k + u) & 15
-                  v0 = fmaf(W[(15 - k + u) & 15], T[k], v0);
-                  v1 = fmaf(W[(14 - k + u) & 15], T[k + 1], v1);
+          for (int u = 0; u < UP_RUN; ++u) {
+            const int c0 = cbase + 2 * u;
+            if (u < nrun) {
+              if (c0 >= 0 && c0 < wout) out[c0][lane] = X[u + 7];          // phase 0: the copy of Eq. 8 case 1
+              if (c0 + 1 >= 0 && c0 + 1 < wout) out[c0 + 1][lane] = odd[u];
+            }
+          }
+        }
+      } else {
+        const float *g = uptaps + uptap_off[lf];
+#pragma unroll
+        for (int u = 0; u < UP_RUN; ++u) {
+          if (u < nrun) {
+            for (int ph = 0; ph < f; ++ph) {
+              float v0 = 0.f, v1 = 0.f;
+              if (ph == 0) v0 = X[u + 7];
+              else {
+#pragma unroll
+                for (int k = 0; k < 16; k += 2) {
+                  v0 = fmaf(X[u + 15 - k], g[k * f + ph], v0);
+                  v1 = fmaf(X[u + 14 - k], g[(k + 1) * f + ph], v1);
                 }
-                const float v = v0 + v1;
-                if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v); }
-                else out[c][lane] = v;
               }
-            } else {
-              for (int ph = 1; ph < f; ++ph) {
-                const int c = c0 + ph;
-                if (c >= 0 && c < wout) {
-                  float v0 = 0.f, v1 = 0.f;
-#pragma unroll
-                  for (int k = 0; k < 16; k += 2) {
-                    v0 = fmaf(W[(15 - k + u) & 15], g[k * f + ph], v0);
-                    v1 = fmaf(W[(14 - k + u) & 15], g[(k + 1) * f + ph], v1);
-                  }
-                  const float v = v0 + v1;
-                  if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v); }
-                  else out[c][lane] = v;
-                }
+              const int c = cbase + (u << lf) + ph;
+              if (c >= 0 && c < wout) {
+                if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v0 + v1); }
+                else out[c][lane] = v0 + v1;
               }
             }
           }
@@ -229,9 +258,18 @@ __global__ void __launch_bounds__(256) upsample_kernel(const UpItem *__restrict_
 cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
                             const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
-  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0);
-  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0);
-  else upsample_kernel<2><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0);
+  static UpTaps2 t2;                                     // Eq. 4 with f = 2, c = 16 (same float64 -> fp32 values as uptaps)
+  static bool have = false;
+  if (!have) {
+    for (int k = 0; k < 16; ++k) {
+      const double x = (2 * k + 1) - 16.0, a = M_PI * x / 2.0, b = M_PI * x / 16.0;
+      t2.t[k] = (float)((sin(a) / a) * (sin(b) / b));
+    }
+    have = true;
+  }
+  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else upsample_kernel<2><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
   return cudaGetLastError();
 }
 
