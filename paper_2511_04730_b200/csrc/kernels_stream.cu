@@ -31,50 +31,61 @@ __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, cons
     }
     return;
   }
-  // DEC_PER_CTA consecutive (flattened) outputs per CTA; the 256 threads split the taps of each output, partial
+  // DEC_PER_CTA consecutive outputs of ONE rate per CTA (out_begin is padded to a multiple of DEC_PER_CTA).  The 256
+  // threads split the taps; each thread carries all DEC_PER_CTA accumulators so its loads are independent.  Partial
   // sums are reduced in a fixed order (lane tree, then warps 0..7): deterministic.
   __shared__ float part[DEC_PER_CTA][8];
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int o0 = (blockIdx.x - P.copy_blocks) * DEC_PER_CTA;
-#pragma unroll 1
-  for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
-    const int o = o0 + oi;
-    if (o >= P.total_out) break;
-    int ri = 1;
-    while (ri + 1 < P.n_rates && o >= P.r[ri + 1].out_begin) ++ri;
-    const RateDev &r = P.r[ri];
-    const long long j = n0 / r.D - r.lag + (o - r.out_begin);
-    const long long top = j * r.D + r.c;            // f0 index read by tap k = 0
-    float acc = 0.f;
-    const int ntap = 2 * r.c + 1;
-    for (int k = threadIdx.x; k < ntap; k += 256) {
-      long long i = top - k;
-      float v;
-      if (i >= n0) v = sd[i - n0];
-      else if (i < 0) v = 0.f;
-      else v = ring0[(int)(i % r0.rlen)];
-      acc = fmaf(r.taps[k], v, acc);
-    }
+  if (o0 >= P.total_out) return;
+  int ri = 1;
+  while (ri + 1 < P.n_rates && o0 >= P.r[ri + 1].out_begin) ++ri;
+  const RateDev &r = P.r[ri];
+  const int first = o0 - r.out_begin;                      // first output of this CTA within the push
+  if (first >= r.n_out) return;
+  const long long j0 = n0 / r.D - r.lag + first;
+  const long long top0 = j0 * r.D + r.c;                   // f0 index read by tap k = 0 of output j0
+  const int ntap = 2 * r.c + 1, D = r.D, rlen0 = r0.rlen;
+  const float *__restrict__ taps = r.taps;
+  float acc[DEC_PER_CTA];
 #pragma unroll
-    for (int s = 16; s > 0; s >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, s);
-    if (lane == 0) part[oi][warp] = acc;
+  for (int oi = 0; oi < DEC_PER_CTA; ++oi) acc[oi] = 0.f;
+  // strain index of (output oi, tap k): top0 + oi*D - k; below n0 it lives in the f0 ring, below 0 it is zero
+  const long long rel0 = top0 - n0;                        // index relative to the pushed buffer (may be negative)
+  int ring_base = (int)(((n0 % rlen0) + rlen0) % rlen0);   // ring slot of stream sample n0
+  for (int k = threadIdx.x; k < ntap; k += 256) {
+    const float t = taps[k];
+#pragma unroll
+    for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
+      const long long rel = rel0 + (long long)oi * D - k;
+      float v;
+      if (rel >= 0) v = sd[rel];
+      else if (rel + n0 < 0) v = 0.f;
+      else {
+        long long sl = ring_base + rel;                    // rel in (-rlen0, 0): one wrap at most
+        if (sl < 0) sl += rlen0;
+        v = ring0[sl];
+      }
+      acc[oi] = fmaf(t, v, acc[oi]);
+    }
+  }
+#pragma unroll
+  for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
+    float a = acc[oi];
+#pragma unroll
+    for (int s = 16; s > 0; s >>= 1) a += __shfl_xor_sync(0xffffffffu, a, s);
+    if (lane == 0) part[oi][warp] = a;
   }
   __syncthreads();
-  if (threadIdx.x < DEC_PER_CTA) {
-    const int o = o0 + threadIdx.x;
-    if (o < P.total_out) {
-      int ri = 1;
-      while (ri + 1 < P.n_rates && o >= P.r[ri + 1].out_begin) ++ri;
-      const RateDev &r = P.r[ri];
-      const long long j = n0 / r.D - r.lag + (o - r.out_begin);
-      float acc = 0.f;
+  if (threadIdx.x < DEC_PER_CTA && first + (int)threadIdx.x < r.n_out) {
+    const long long j = j0 + threadIdx.x;
+    float a = 0.f;
 #pragma unroll
-      for (int w = 0; w < 8; ++w) acc += part[threadIdx.x][w];
-      int slot = (int)((j + r.lag) % r.rlen);
-      float *ring = r.ring2 + (size_t)det * 2 * r.rlen;
-      ring[slot] = acc;
-      ring[slot + r.rlen] = acc;
-    }
+    for (int w = 0; w < 8; ++w) a += part[threadIdx.x][w];
+    int slot = (int)((j + r.lag) % r.rlen);
+    float *ring = r.ring2 + (size_t)det * 2 * r.rlen;
+    ring[slot] = a;
+    ring[slot + r.rlen] = a;
   }
 }
 

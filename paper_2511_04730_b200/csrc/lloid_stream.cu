@@ -143,7 +143,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       std::vector<float> t(g.size());
       for (size_t k = 0; k < g.size(); ++k) t[k] = (float)(std::sqrt((double)D) * g[k] / sum);
       float *td; CK(dev_upload(s, &td, t)); r.taps = td;
-      r.out_begin = out_begin; out_begin += r.n_out;
+      r.out_begin = out_begin; out_begin += (r.n_out + 7) / 8 * 8;   // groups of 8 outputs never straddle rates
     }
   }
   dp.total_out = out_begin;
