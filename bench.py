@@ -36,7 +36,7 @@ def parse():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); default 2 = configs[1]")
-    ap.add_argument("--precision", default=os.environ.get("LLOID_BENCH_PRECISION", "ffma"), choices=list(PREC))
+    ap.add_argument("--precision", default=os.environ.get("LLOID_BENCH_PRECISION", "split"), choices=list(PREC))
     ap.add_argument("--banks", type=int, default=0, help="debug: use only the first n banks (0 = all; marks the run as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-flush", action="store_true", help="keep L2 warm between steps (reported in config)")
@@ -46,13 +46,81 @@ def parse():
 # ---------------------------------------------------------------------------------------------------------
 # workload
 # ---------------------------------------------------------------------------------------------------------
-def build_workload(cfg_no, n_banks_limit, seconds, rank=0):
-    """Banks (float32-rounded SVD banks of the config) and [n_det][seconds*f0] strain, seeded (DESIGN.md recipe)."""
-    from workloads import CONFIGS, make_strain
+N_REAL_BANKS = 4        # configs with many banks: this many real chirp-SVD banks, the rest shape-faithful stand-ins
+
+
+def _real_bank(args):
+    """One chirp-SVD bank of the config.  Generation is deterministic and slow for 1000-template banks (0.5-2 min),
+    so the result is memoised under /tmp (an input cache only: a miss just recomputes the same arrays)."""
+    cfg_no, b = args
+    import pickle
+    from workloads import CONFIGS
+    c = CONFIGS[cfg_no]
+    path = os.path.join("/tmp", "lloid_bank_cache", f"seed{c.seed(999)}_M{c.M}_nb{c.n_banks}_T{int(c.T_max)}_b{b}.pkl")
+    try:
+        with open(path, "rb") as f:
+            return b, pickle.load(f)
+    except Exception:
+        pass
+    bank = c.bank(b, method="gram" if c.M >= 1000 else "svd").as_f32()
+    try:
+        os.makedirs(os.path.dirname(path), exist_ok=True)
+        with open(path + f".{os.getpid()}", "wb") as f:
+            pickle.dump(bank, f, protocol=4)
+        os.replace(path + f".{os.getpid()}", path)
+    except Exception:
+        pass
+    return b, bank
+
+
+def bank_plan(cfg_no, n_banks_limit):
+    """(config, list of bank descriptions).  Configs 1-2: every bank is the config's chirp-SVD bank.  Configs 3-5
+    (100-1000 banks; one SVD bank takes 0.5-1 min of host time): N_REAL_BANKS evenly spaced real banks; every other
+    bank keeps its REAL slice layout (rates, taps, delays from its own chirp masses) and takes the basis counts L^s of
+    the nearest real bank, with seeded random orthonormal U and random R (SURVEY.md section 8d "scale handling")."""
+    from workloads import CONFIGS
+    c = CONFIGS[cfg_no]
+    nb = c.n_banks if not n_banks_limit else min(n_banks_limit, c.n_banks)
+    if nb <= 8:
+        return c, [("real", b) for b in range(nb)]
+    real = sorted(set(int(round(i * (nb - 1) / (N_REAL_BANKS - 1))) for i in range(N_REAL_BANKS)))
+    return c, [("real", b) if b in real else ("standin", b, min(real, key=lambda r: abs(r - b))) for b in range(nb)]
+
+
+def iter_banks(cfg_no, plan, describe=None):
+    """Yield the planned banks one at a time (the caller uploads each and drops it)."""
+    import multiprocessing as mp
+    from workloads import CONFIGS, random_bank
     c = CONFIGS[cfg_no]
     mcs = c.mchirps()
-    nb = c.n_banks if not n_banks_limit else min(n_banks_limit, c.n_banks)
-    banks = [c.bank(b, method="gram" if c.M >= 1000 else "svd", mcs=mcs).as_f32() for b in range(nb)]
+    real_ids = [p[1] for p in plan if p[0] == "real"]
+    if len(real_ids) > 1 and c.M >= 1000:
+        with mp.get_context("fork").Pool(min(len(real_ids), os.cpu_count() or 1)) as pool:
+            real = dict(pool.map(_real_bank, [(cfg_no, b) for b in real_ids]))
+    else:
+        real = dict(_real_bank((cfg_no, b)) for b in real_ids)
+    for p in plan:
+        if p[0] == "real":
+            bank = real[p[1]]
+        else:
+            _, b, src = p
+            T, lay = c.layout(b, mcs)
+            Ls = [s.n_basis for s in real[src].slices]
+            shape = [(rate, (e - s0) // (c.f0 // rate), Ls[min(i, len(Ls) - 1)]) for i, (rate, s0, e) in enumerate(lay)]
+            bank = random_bank(c.seed(b), c.M, shape, f0=c.f0).as_f32()
+        if describe is not None:
+            describe.append(("real " if p[0] == "real" else "standin ") + bank.describe())
+        yield bank
+
+
+def build_workload(cfg_no, n_banks_limit, seconds, rank=0, only_real=True):
+    """Banks (float32-rounded) and [n_det][seconds*f0] strain, seeded (DESIGN.md "Input recipe").  only_real: for the
+    many-bank configs return just the real chirp-SVD banks (what the oracle legs sample)."""
+    from workloads import make_strain
+    c, plan = bank_plan(cfg_no, n_banks_limit)
+    if only_real:
+        plan = [p for p in plan if p[0] == "real"]
+    banks = list(iter_banks(cfg_no, plan))
     # white N(0,1) strain per detector; ranks > 0 (weak scaling replicas) shift the detector seeds
     strain = np.stack([make_strain(c.seed(det) + 100 * rank, seconds * c.f0) for det in range(c.n_det)])
     return c, banks, strain
@@ -187,15 +255,34 @@ def run_ours(args):
 
     K, W = args.steps, args.warmup
     n_total = 3 * K + W                        # device-timed K, end-to-end K, stage-timed K
-    c, banks, strain = build_workload(args.config, args.banks, n_total, rank)
+    from workloads import make_strain
+    c, plan = bank_plan(args.config, args.banks)
     B, f0 = c.buffer_len, c.f0
-    st = lib.LloidStream(banks, c.n_det, B, precision=PREC[args.precision], device=f"cuda:{local_rank}")
+    descr = []
+    keep = []                                  # banks kept on the host only when the oracle baseline needs them
+    def gen():
+        for bank in iter_banks(args.config, plan, descr):
+            if descr[-1].startswith("real"):
+                keep.append(bank)
+            yield bank
+    st = lib.LloidStream(gen(), c.n_det, B, precision=PREC[args.precision], device=f"cuda:{local_rank}")
+    banks = keep
+    n_seconds = -(-n_total * B // f0)
+    strain = np.stack([make_strain(c.seed(det) + 100 * rank, n_seconds * f0) for det in range(c.n_det)])[:, :n_total * B]
     units_per_step = st.Mtot * c.n_det * (B / f0)
     pool = torch.from_numpy(strain.reshape(c.n_det, n_total, B).transpose(1, 0, 2).copy()).to(dev)   # [step][det][B]
-    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev)        # 256 MiB > 126 MB L2
+    work = st.work_per_push()
+    # L2 policy: the operands (U, R) and intermediates one push touches either exceed the 126 MB L2 several times
+    # over (configs 3-5) or the L2 is flushed between steps by writing 256 MiB (configs 1-2)
+    touched = work[5] + work[6] / 2
+    do_flush = (not args.no_flush) and touched < 4 * 126e6
+    flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if do_flush else None
+    l2_note = ("flushed between steps (256 MiB memset, untimed)" if do_flush else
+               ("warm (--no-flush)" if args.no_flush and touched < 4 * 126e6 else
+                f"not flushed: one push touches {touched / 1e6:.0f} MB of operands/intermediates (> 4x the 126 MB L2)"))
 
     def flush():
-        if not args.no_flush:
+        if do_flush:
             flush_buf.zero_()
 
     step = 0
@@ -210,10 +297,13 @@ def run_ours(args):
         dist.barrier()
     torch.cuda.synchronize()
     wall0 = time.perf_counter()
+    host_ms = []
     for i in range(K):                                                        # ---- device-timed region
         flush()
         ev0[i].record()
+        h0 = time.perf_counter()
         st.push_device(pool[step]); step += 1
+        host_ms.append(1e3 * (time.perf_counter() - h0))
         ev1[i].record()
     torch.cuda.synchronize()
     if world > 1:
@@ -240,17 +330,17 @@ def run_ours(args):
         flush(); st.push_device(pool[step]); step += 1
     n_cov, stage_ms = st.stage_times()
     st.set_stage_timing(False)
-    work = st.work_per_push()
     launches = st.launches_per_push
     st.close()
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
         return
-    line = assemble(args, c, banks, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks)
-    if not args.no_cpu_baseline and world == 1:
+    line = assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
+                    l2_note, host_ms)
+    if not args.no_cpu_baseline and world == 1 and banks:
         hist_s = 4
-        _, _, strain_o = build_workload(args.config, args.banks, hist_s + 1)
+        strain_o = np.stack([make_strain(c.seed(det), (hist_s + 1) * f0) for det in range(c.n_det)])[:, :hist_s * f0 + B]
         v, s_per, sample = time_oracle(banks, strain_o, B, f0, 15.0, 1, 0)
         line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample}
     print(json.dumps(line), flush=True)
@@ -266,7 +356,8 @@ def measured_peaks():
     return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
 
-def assemble(args, c, banks, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks):
+def assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
+             l2_note, host_ms):
     peaks, peak_src = measured_peaks()
     value = whole_job_value(world, units_per_step, K, t_dev)
     e2e = whole_job_value(world, units_per_step, K, t_e2e)
@@ -305,19 +396,26 @@ def assemble(args, c, banks, world, K, W, units_per_step, t_dev, ms, wall, t_e2e
     roof["stage_ms_per_push"] = per_stage
     roof["stage_share"] = {k: v / max(sum(per_stage.values()), 1e-12) for k, v in per_stage.items()}
     reduced = bool(args.banks) and args.banks < c.n_banks
+    banks = descr
     return {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
         "ms_per_step": 1e3 * t_dev / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
         "dtype": PREC_DTYPE[args.precision], "data": "synthetic",
         "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({c.name})" + (" REDUCED (--banks)" if reduced else ""),
-                   "n_banks": len(banks), "templates_per_bank": c.M, "n_detectors": c.n_det, "buffer_len": c.buffer_len,
-                   "slices": [b.describe() for b in banks[:4]], "precision": args.precision,
-                   "l2": "warm (--no-flush)" if args.no_flush else "flushed between steps (256 MiB memset, untimed)",
+                   "n_banks": len(descr), "templates_per_bank": c.M, "n_detectors": c.n_det, "buffer_len": c.buffer_len,
+                   "banks": (f"{sum(d.startswith('real') for d in descr)} chirp-SVD banks + "
+                             f"{sum(d.startswith('standin') for d in descr)} shape-faithful stand-ins (real slice layout, L^s of the "
+                             "nearest SVD bank, random orthonormal U / random R)"),
+                   "slices": descr[:2] + descr[-2:], "precision": args.precision, "l2": l2_note,
                    "timing": "sum of per-step CUDA-event intervals (push only), max over ranks",
                    "multi_gpu": "independent replicas of the workload, no data-path collective"},
         "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": c.n_det * c.buffer_len * 4,
-                "d2h_bytes_per_step": int(c.n_det * sum(b.M for b in banks) * 12), "ms_per_step": 1e3 * t_e2e / K},
+                "d2h_bytes_per_step": int(c.n_det * len(descr) * c.M * 12), "ms_per_step": 1e3 * t_e2e / K},
         "gpu_launches": launches * K, "wall_ms_timed_region": 1e3 * wall, "ms_step_min_med_max": [min(ms), float(np.median(ms)), max(ms)],
+        "latency_ms": {"device_p50": float(np.percentile(ms, 50)), "device_p99": float(np.percentile(ms, 99)),
+                       "device_max": max(ms), "host_launch_p50": float(np.percentile(host_ms, 50)),
+                       "host_launch_p99": float(np.percentile(host_ms, 99)),
+                       "note": "per-push device time (CUDA events around one lloid_stream_push) and host time of the call"},
         "clocks": clocks, "roofline": roof,
     }
 

@@ -205,8 +205,10 @@ class LloidStream:
         self.device = torch.device(device)
         torch.cuda.set_device(self.device)
         self.n_det, self.B = n_detectors, buffer_len
-        self.Ms = [b.M for b in banks]
-        self.bank_handles = [lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold) for b in banks]
+        self.Ms, self.bank_handles = [], []
+        for b in banks:                      # any iterable: a generator lets the caller build banks one at a time
+            self.Ms.append(b.M)
+            self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold))
         self.cuda_stream = torch.cuda.current_stream(self.device)
         self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
         self.Mtot = lloid_stream_total_templates(self.handle)
