@@ -152,6 +152,13 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   const bool active = lane < it->nl;
   const int ylen = it->ylen, ypitch = it->ypitch, kpitch = it->kpitch;
   const float *yr = it->yring + (size_t)det * it->ydet_stride + it->row0 + lane;
+  const int nseg = it->nseg;
+  const size_t yseg = (size_t)it->yseg_stride;
+  auto load_y = [&](int sl) {                              // split-K partial sums added in segment order
+    float v = yr[(size_t)sl * ypitch];
+    for (int sg = 1; sg < nseg; ++sg) v += yr[sg * yseg + (size_t)sl * ypitch];
+    return v;
+  };
   void *yup = it->yup;
   const size_t plane_stride = (size_t)it->yup_plane_stride;
   const size_t out0 = (size_t)det * it->yup_det_stride + (size_t)it->kcol + lane + (size_t)ka * kpitch;   // sample ka
@@ -165,7 +172,7 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
       float v[4];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        v[i] = (active && c + i * nwarp < wg) ? yr[(size_t)slot * ypitch] : 0.f;
+        v[i] = (active && c + i * nwarp < wg) ? load_y(slot) : 0.f;
         slot += nwarp; if (slot >= ylen) slot -= ylen;
       }
 #pragma unroll
@@ -178,7 +185,7 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
     float v[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      v[i] = (active && c + i * nwarp < wg) ? yr[(size_t)slot * ypitch] : 0.f;
+      v[i] = (active && c + i * nwarp < wg) ? load_y(slot) : 0.f;
       slot += nwarp; if (slot >= ylen) slot -= ylen;
     }
 #pragma unroll

@@ -31,7 +31,6 @@ struct TcReconBank {                         // device copy, 64-byte aligned (CU
   float inv_scale;
   int pad_[11];
 };
-struct TcCorrTile { int cls, det, row0, col0; };
 struct TcCorrClass {
   CUtensorMap mapU;                          // [planes*Lpad rows][Npad] fp16, box 64 x 128
   int pad_[32];
@@ -73,7 +72,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
         const TcReconTile tl = tiles[ti];
         const TcReconBank *bk = &banks[tl.bank];
-        const int nkb = bk->Kpad / BK;
+        const int nkb = (bk->Kpad + BK - 1) / BK;
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(&empty[stage], phase ^ 1);
           mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
@@ -95,7 +94,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       int stage = 0; uint32_t phase = 0; int it = 0;
       for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x, ++it) {
         const TcReconTile tl = tiles[ti];
-        const int nkb = banks[tl.bank].Kpad / BK;
+        const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
         const int buf = it & 1;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
@@ -104,8 +103,10 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           mbar_wait(&full[stage], phase);
           tc_fence_after_sync();
           const uint32_t s = smem_u32(smem + stage * STAGE_BYTES);
+          const int nk = min(BK / 16, (Kpad - kb * BK) / 16);       // K is padded to 16, the last 64-wide box is zero-filled
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) {
+            if (k >= nk) break;
             const uint32_t ko = k * 32;
             const bool acc = (kb | k) != 0;
             const uint64_t re_hi = desc_kmajor_sw128(s + 0 * TILE_BYTES + ko), im_hi = desc_kmajor_sw128(s + 1 * TILE_BYTES + ko),
@@ -172,161 +173,223 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 }
 
 // ------------------------------------------------------------------------------------------------
-// a2.  One tile per CTA (2 CTAs per SM): 128 stacked basis rows x NT <= 128 columns of one (class, detector);
-// K = the slice's taps, walked in chunks of KS = 512.  For each chunk warps 2-5 build the Hankel strip
-//   strip[m][r][e] = x[c*KS + 8 m + r + e]   (fp16; m < (NT + ks)/8, r < 8, e < 8; 128 B per m)
-// from the fp32 strain ring, so that B[n][k] = x[n + k] is the no-swizzle K-major operand with
-// LBO = SBO = 128 B starting at strip + 128*(k/8) bytes.  U tiles come by TMA.  The accumulator
-// [128 x NT] fp32 sits in 128 TMEM columns; the epilogue scales and writes the Y ring (time-major).
+// a2.  Persistent CTAs (one per SM) over work UNITS = (class, 128 stacked basis rows, tap segment of <= 1024 taps,
+// up to 4 sub-tiles), a sub-tile being 128 (or fewer) output columns of one detector.  All sub-tiles of a unit share
+// the U tiles (read once from L2 for up to 512 output columns); the tap segments (split K) of a slice balance the
+// load and their partial sums go to separate planes of the Y ring, added in order by the reader (deterministic).
+// For each chunk of KS = 128 taps warps 2-5 build, per sub-tile, the Hankel strip
+//   strip[m][r][e] = x[k + 8 m + r + e]   (fp16; m < (NT + KS)/8, r < 8, e < 8; 128 B per m)
+// from the strain window staged in shared memory, so that B[n][k] = x[n + k] is a no-swizzle K-major operand with
+// LBO = SBO = 128 B starting at strip + 16*k bytes.  Accumulators: 4 x [128 x 128] fp32 = all 512 TMEM columns.
 // ------------------------------------------------------------------------------------------------
-static constexpr int KS = 512;
-static constexpr int STRIP_BYTES = (TILE_N + KS) * 16;        // one plane, one buffer: 10240 B
+static constexpr int KS = 128;                                // taps per strip chunk (2 U stages)
+static constexpr int KSEG_MAX = 1024;                         // taps per unit (split-K segment)
+static constexpr int MAX_SUB = 2;
+static constexpr int STRIP_BYTES = (TILE_N + KS) * 16;        // one sub-tile, one plane, one buffer: 4096 B
+static constexpr int XWIN = TILE_N + KSEG_MAX + 8;            // staged strain window per sub-tile (floats)
+static constexpr int CORR_THREADS = 320;                      // warps: 0 TMA, 1 MMA, 2-5 epilogue, 6-9 strip builders
+
+struct TcCorrUnit {
+  int cls, row0, k0, k1;                                      // taps [k0, k1), multiples of 64
+  int seg, nsub;
+  int det[MAX_SUB], col0[MAX_SUB];
+};
+
+int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
 
 template <int PLANES>
-__global__ void __launch_bounds__(TC_THREADS, 2)
-corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restrict__ maps, const TcCorrTile *__restrict__ tiles,
-               const long long *__restrict__ n0_ptr) {
-  constexpr int STAGES = 2;
+__global__ void __launch_bounds__(CORR_THREADS, 1)
+corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restrict__ maps, const TcCorrUnit *__restrict__ units,
+               int n_units, const long long *__restrict__ n0_ptr) {
+  constexpr int STAGES = PLANES == 2 ? 4 : 6;
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t *strips = smem + STAGES * STAGE_BYTES;                 // [2 buffers][PLANES][STRIP_BYTES]
-  uint64_t *bars = (uint64_t *)(strips + 2 * PLANES * STRIP_BYTES);
-  uint64_t *ufull = bars, *uempty = bars + STAGES, *sfull = bars + 2 * STAGES, *sempty = sfull + 2, *accfull = sempty + 2;
-  uint32_t *tmem_slot = (uint32_t *)(accfull + 1);
+  uint8_t *strips = smem + STAGES * STAGE_BYTES;                 // [2 buffers][MAX_SUB][PLANES][STRIP_BYTES]
+  float *xwin = (float *)(strips + 2 * MAX_SUB * PLANES * STRIP_BYTES);   // [MAX_SUB][XWIN]
+  uint64_t *bars = (uint64_t *)(xwin + MAX_SUB * XWIN);
+  uint64_t *ufull = bars, *uempty = bars + STAGES, *sfull = bars + 2 * STAGES, *sempty = sfull + 2, *tfull = sempty + 2,
+           *tempty = tfull + 2;
+  uint32_t *tmem_slot = (uint32_t *)(tempty + 2);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-  const TcCorrTile tl = tiles[blockIdx.x];
-  const CorrClass &c = classes[tl.cls];
-  const int NT = min(TILE_N, (c.ncols - tl.col0 + 15) & ~15);    // MMA N: multiple of 16
-  const int nkb = c.Npad / BK;                                   // 64-tap blocks
-  const int nchunk = (c.Npad + KS - 1) / KS;
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&ufull[i], 1); mbar_init(&uempty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&sfull[i], 4); mbar_init(&sempty[i], 1); }
-    mbar_init(accfull, 1);
+    for (int i = 0; i < 2; ++i) { mbar_init(&sfull[i], 4); mbar_init(&sempty[i], 1); mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4); }
     mbar_fence_init();
   }
-  if (warp == 1) tmem_alloc(tmem_slot, 128);
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
   tc_fence_before_sync();
   __syncthreads();
   tc_fence_after_sync();
   const uint32_t tmem = *tmem_slot;
 
   if (warp == 0) {
+    // ===== TMA producer: U tiles of 128 rows x 64 taps (x planes), in unit order
     if (lane == 0) {
-      const CUtensorMap *mapU = &maps[tl.cls].mapU;
       int stage = 0; uint32_t phase = 0;
-      for (int kb = 0; kb < nkb; ++kb) {
-        mbar_wait(&uempty[stage], phase ^ 1);
-        mbar_arrive_expect_tx(&ufull[stage], STAGE_BYTES);
+      for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x) {
+        const TcCorrUnit *u = &units[ui];
+        const CUtensorMap *mapU = &maps[u->cls].mapU;
+        const int Lpad = classes[u->cls].Lpad, row0 = u->row0, k1 = u->k1;
+        for (int k = u->k0; k < k1; k += BK) {
+          mbar_wait(&uempty[stage], phase ^ 1);
+          mbar_arrive_expect_tx(&ufull[stage], STAGE_BYTES);
 #pragma unroll
-        for (int p = 0; p < PLANES; ++p)
-          tma_load_2d(smem + stage * STAGE_BYTES + p * TILE_BYTES, mapU, &ufull[stage], kb * BK, p * c.Lpad + tl.row0);
-        if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          for (int p = 0; p < PLANES; ++p)
+            tma_load_2d(smem + stage * STAGE_BYTES + p * TILE_BYTES, mapU, &ufull[stage], k, p * Lpad + row0);
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+        }
       }
     }
   } else if (warp == 1) {
+    // ===== MMA issuer.  Descriptors differ only in their 14-bit address field (16-byte units): one 64-bit add each.
     if (lane == 0) {
-      const uint32_t idesc = idesc_f16_f32(TILE_M, NT);
-      int stage = 0; uint32_t phase = 0;
-      for (int ch = 0; ch < nchunk; ++ch) {
-        const int sb = ch & 1;
-        mbar_wait(&sfull[sb], (ch >> 1) & 1);
+      int stage = 0; uint32_t phase = 0; int it = 0, chunk_it = 0;
+      for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x, ++it) {
+        const TcCorrUnit *u = &units[ui];
+        const int nsub = u->nsub, ncols = classes[u->cls].ncols, k0 = u->k0, k1 = u->k1;
+        const uint32_t idesc0 = idesc_f16_f32(TILE_M, min(TILE_N, (ncols - u->col0[0] + 15) & ~15));
+        const uint32_t idesc1 = idesc_f16_f32(TILE_M, nsub > 1 ? min(TILE_N, (ncols - u->col0[1] + 15) & ~15) : 16);
+        const int buf = it & 1;
+        mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
-        const uint32_t strip = smem_u32(strips + sb * PLANES * STRIP_BYTES);
-        const int kb_end = min(nkb, (ch + 1) * (KS / BK));
-        for (int kb = ch * (KS / BK); kb < kb_end; ++kb) {
-          mbar_wait(&ufull[stage], phase);
+        const uint32_t d0 = tmem + buf * (MAX_SUB * TILE_N), d1 = d0 + TILE_N;
+        for (int kc = k0; kc < k1; kc += KS, ++chunk_it) {
+          const int sbuf = chunk_it & 1;
+          mbar_wait(&sfull[sbuf], (chunk_it >> 1) & 1);
           tc_fence_after_sync();
-          const uint32_t us = smem_u32(smem + stage * STAGE_BYTES);
+          const uint64_t xd = desc_kmajor_nosw(smem_u32(strips + sbuf * MAX_SUB * PLANES * STRIP_BYTES), 128, 128);
+          const int kend = min(kc + KS, k1);
+          for (int kb = kc; kb < kend; kb += BK) {
+            mbar_wait(&ufull[stage], phase);
+            tc_fence_after_sync();
+            const uint64_t ud = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
+            const uint64_t xk = xd + (uint64_t)(kb - kc);              // 16 B per tap
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k) {
-            const uint32_t koff = (uint32_t)((kb - ch * (KS / BK)) * BK + k * 16) * 16;   // 128 B per 8 taps
-            const uint64_t u_hi = desc_kmajor_sw128(us + k * 32);
-            const uint64_t x_hi = desc_kmajor_nosw(strip + koff, 128, 128);
-            mma_f16_ss(tmem, u_hi, x_hi, idesc, (kb | k) != 0);
-            if (PLANES == 2) {
-              const uint64_t u_lo = desc_kmajor_sw128(us + TILE_BYTES + k * 32);
-              const uint64_t x_lo = desc_kmajor_nosw(strip + STRIP_BYTES + koff, 128, 128);
-              mma_f16_ss(tmem, u_hi, x_lo, idesc, true);
-              mma_f16_ss(tmem, u_lo, x_hi, idesc, true);
+            for (int k = 0; k < BK / 16; ++k) {
+              const bool acc = (kb > k0) || (k > 0);
+              const uint64_t u_hi = ud + 2 * k, u_lo = u_hi + (TILE_BYTES >> 4);
+              const uint64_t x0_hi = xk + 16 * k, x0_lo = x0_hi + (STRIP_BYTES >> 4);
+              mma_f16_ss(d0, u_hi, x0_hi, idesc0, acc);
+              if (PLANES == 2) { mma_f16_ss(d0, u_hi, x0_lo, idesc0, true); mma_f16_ss(d0, u_lo, x0_hi, idesc0, true); }
+              if (nsub > 1) {
+                const uint64_t x1_hi = x0_hi + (PLANES * STRIP_BYTES >> 4), x1_lo = x1_hi + (STRIP_BYTES >> 4);
+                mma_f16_ss(d1, u_hi, x1_hi, idesc1, acc);
+                if (PLANES == 2) { mma_f16_ss(d1, u_hi, x1_lo, idesc1, true); mma_f16_ss(d1, u_lo, x1_hi, idesc1, true); }
+              }
             }
+            mma_commit(&uempty[stage]);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
-          mma_commit(&uempty[stage]);
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          mma_commit(&sempty[sbuf]);
         }
-        mma_commit(&sempty[sb]);
+        mma_commit(&tfull[buf]);
       }
-      mma_commit(accfull);
+    }
+  } else if (warp >= 6) {
+    // ===== strip builders (128 threads): stage the strain windows of a unit, then build its strips chunk by chunk
+    const int tid = threadIdx.x - 192;
+    const long long n0 = *n0_ptr;
+    int chunk_it = 0;
+    for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x) {
+      const TcCorrUnit *u = &units[ui];
+      const CorrClass &c = classes[u->cls];
+      const int nsub = u->nsub, k0 = u->k0, klen = u->k1 - k0;
+      asm volatile("bar.sync 1, 128;" ::: "memory");             // every builder is done with the previous unit's windows
+      for (int sb = 0; sb < nsub; ++sb) {
+        // sub-tile sb needs x[first + k0 + i], i in [0, NT + klen): contiguous in the mirrored ring
+        const long long first = n0 / c.D + c.H + u->col0[sb] - c.delay - c.N + 1 + c.lag;
+        const int p0 = (int)(((first % c.rlen) + c.rlen) % c.rlen);
+        const float *x = c.ring2 + (size_t)u->det[sb] * c.ring_det_stride + p0 + k0;
+        float *w = xwin + sb * XWIN;
+        const int nw = TILE_N + klen + 8;
+        for (int i = tid; i < nw; i += 4 * 128) {
+          float v[4];
+#pragma unroll
+          for (int j = 0; j < 4; ++j) v[j] = (i + j * 128 < nw) ? x[i + j * 128] : 0.f;
+#pragma unroll
+          for (int j = 0; j < 4; ++j) if (i + j * 128 < nw) w[i + j * 128] = v[j];
+        }
+      }
+      asm volatile("bar.sync 1, 128;" ::: "memory");
+      for (int kc = 0; kc < klen; kc += KS, ++chunk_it) {
+        const int sbuf = chunk_it & 1;
+        mbar_wait(&sempty[sbuf], ((chunk_it >> 1) & 1) ^ 1);
+        const int n_ent = TILE_N + min(KS, klen - kc);            // entry e = 8 m + r holds x[kc + e .. kc + e + 8)
+        for (int sb = 0; sb < nsub; ++sb) {
+          uint8_t *dst = strips + (sbuf * MAX_SUB + sb) * PLANES * STRIP_BYTES;
+          const float *xs = xwin + sb * XWIN + kc;
+          for (int e = tid; e < n_ent; e += 128) {
+            float v[8];
+#pragma unroll
+            for (int i = 0; i < 8; ++i) v[i] = xs[e + i];
+            __half2 h[4], l[4];
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              h[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+              if (PLANES == 2) {
+                float2 bb = __half22float2(h[i]);
+                l[i] = __floats2half2_rn(v[2 * i] - bb.x, v[2 * i + 1] - bb.y);
+              }
+            }
+            *reinterpret_cast<uint4 *>(dst + (size_t)e * 16) = *reinterpret_cast<uint4 *>(h);
+            if (PLANES == 2) *reinterpret_cast<uint4 *>(dst + STRIP_BYTES + (size_t)e * 16) = *reinterpret_cast<uint4 *>(l);
+          }
+        }
+        fence_proxy_async_smem();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&sfull[sbuf]);
+      }
     }
   } else {
-    // ===== strip builders, then epilogue (128 threads)
-    const int tid = threadIdx.x - 64;
+    // ===== epilogue (warps 2-5): thread = basis row (TMEM lane); partial sums of this tap segment -> plane `seg` of the Y ring
+    const int q = warp & 3;
     const long long n0 = *n0_ptr;
-    const long long j0 = n0 / c.D + c.H + tl.col0;                   // first column of this tile
-    const long long first = j0 - c.delay - c.N + 1 + c.lag;          // ring index of tap 0 of column j0
-    const int p0 = (int)(((first % c.rlen) + c.rlen) % c.rlen);
-    const float *x = c.ring2 + (size_t)tl.det * c.ring_det_stride + p0;   // mirrored ring: the window is contiguous
-    for (int ch = 0; ch < nchunk; ++ch) {
-      const int sb = ch & 1;
-      mbar_wait(&sempty[sb], ((ch >> 1) & 1) ^ 1);
-      const int ks = min(KS, c.Npad - ch * KS);
-      const int n_ent = NT + ks;                                      // (NT + ks)/8 core matrices x 8 rows
-      uint8_t *dst = strips + sb * PLANES * STRIP_BYTES;
-      const float *xs = x + ch * KS;
-      for (int e = tid; e < n_ent; e += 128) {                        // entry e = 8 m + r holds x[e .. e+8)
-        float v[8];
+    int it = 0;
+    for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x, ++it) {
+      const TcCorrUnit *u = &units[ui];
+      const CorrClass &c = classes[u->cls];
+      const int nsub = u->nsub, buf = it & 1;
+      const int ylen = c.ylen, Lpad = c.Lpad, ncols = c.ncols;
+      const float sc = c.u_scale_inv;
+      const int row = u->row0 + q * 32 + lane;
+      const bool row_ok = row < c.Lstack;
+      mbar_wait(&tfull[buf], (it >> 1) & 1);
+      tc_fence_after_sync();
+      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + buf * (MAX_SUB * TILE_N);
+      for (int sb = 0; sb < nsub; ++sb) {
+        const int col0 = u->col0[sb];
+        float *yr = c.yring + (size_t)u->seg * c.yseg_stride + (size_t)u->det[sb] * c.ydet_stride + row;
+        const int NT = min(TILE_N, (ncols - col0 + 15) & ~15);
+        const int slot0 = (int)((n0 / c.D + c.H + col0 + 64) % ylen);
+        for (int cc = 0; cc < NT; cc += 32) {
+          uint32_t v[32];
+          tmem_ld_32x32(taddr + sb * TILE_N + cc, v);
+          tmem_ld_wait();
 #pragma unroll
-        for (int i = 0; i < 8; ++i) v[i] = xs[e + i];
-        __half2 h[4], l[4];
-#pragma unroll
-        for (int i = 0; i < 4; ++i) {
-          h[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
-          if (PLANES == 2) {
-            float2 b = __half22float2(h[i]);
-            l[i] = __floats2half2_rn(v[2 * i] - b.x, v[2 * i + 1] - b.y);
+          for (int i = 0; i < 32; ++i) {
+            int slot = slot0 + cc + i;
+            if (slot >= ylen) slot -= ylen;
+            if (col0 + cc + i < ncols && row_ok) yr[(size_t)slot * Lpad] = __uint_as_float(v[i]) * sc;
           }
         }
-        *reinterpret_cast<uint4 *>(dst + (size_t)e * 16) = *reinterpret_cast<uint4 *>(h);
-        if (PLANES == 2) *reinterpret_cast<uint4 *>(dst + STRIP_BYTES + (size_t)e * 16) = *reinterpret_cast<uint4 *>(l);
       }
-      fence_proxy_async_smem();
+      tc_fence_before_sync();
       __syncwarp();
-      if (lane == 0) mbar_arrive(&sfull[sb]);
-    }
-    // epilogue
-    mbar_wait(accfull, 0);
-    tc_fence_after_sync();
-    const int q = warp & 3;
-    const int row = tl.row0 + q * 32 + lane;
-    float *yr = c.yring + (size_t)tl.det * c.ydet_stride;
-    const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16);
-    for (int cc = 0; cc < NT; cc += 32) {
-      uint32_t v[32];
-      tmem_ld_32x32(taddr + cc, v);
-      tmem_ld_wait();
-#pragma unroll
-      for (int i = 0; i < 32; ++i) {
-        const int col = tl.col0 + cc + i;
-        if (col < c.ncols && row < c.Lstack) {
-          const int slot = (int)((j0 + cc + i + 64) % c.ylen);
-          yr[(size_t)slot * c.Lpad + row] = __uint_as_float(v[i]) * c.u_scale_inv;
-        }
-      }
+      if (lane == 0) mbar_arrive(&tempty[buf]);
     }
   }
   tc_fence_before_sync();
   __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 128);
+  if (warp == 1) tmem_dealloc(tmem, 512);
 }
 
 // ------------------------------------------------------------------------------------------------ host side
 struct TcPlan {
   int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
-  TcCorrClass *cmaps_dev; TcCorrTile *ctiles_dev; int n_ctiles;
+  TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
   int recon_grid, recon_smem, corr_smem;
   std::vector<void *> allocs;
@@ -390,21 +453,36 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->n_tt = tc_time_splits(B); p->classes_dev = classes_dev;
-  // ---- a2: one tensor map per class, tiles ordered by decreasing K so the long ones start first
+  // ---- a2: one tensor map per class; units = (row tile, tap segment, group of <= 4 (detector, column tile) sub-tiles),
+  //      dealt to the persistent CTAs in order of decreasing cost
   std::vector<TcCorrClass> cm(classes.size());
-  std::vector<TcCorrTile> ct;
-  std::vector<int> order(classes.size());
-  for (size_t i = 0; i < classes.size(); ++i) order[i] = (int)i;
-  std::sort(order.begin(), order.end(), [&](int a, int b) { return classes[a].Npad > classes[b].Npad; });
-  for (int ci : order) {
+  std::vector<TcCorrUnit> cu;
+  for (size_t ci = 0; ci < classes.size(); ++ci) {
     const CorrClass &c = classes[ci];
     memset(&cm[ci], 0, sizeof(TcCorrClass));
     if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    const int nseg = tc_k_segments(c.Npad);
+    const int kseg = ((c.Npad + nseg - 1) / nseg + BK - 1) / BK * BK;
+    std::vector<std::pair<int, int>> subs;
     for (int det = 0; det < n_det; ++det)
-      for (int r0 = 0; r0 < c.Lstack; r0 += TILE_M)
-        for (int c0 = 0; c0 < c.ncols; c0 += TILE_N) ct.push_back({ci, det, r0, c0});
+      for (int c0 = 0; c0 < c.ncols; c0 += TILE_N) subs.push_back({det, c0});
+    for (int r0 = 0; r0 < c.Lstack; r0 += TILE_M)
+      for (int sg = 0; sg < nseg; ++sg) {
+        const int k0 = sg * kseg, k1 = std::min(c.Npad, k0 + kseg);
+        if (k0 >= k1) continue;
+        for (size_t s0 = 0; s0 < subs.size(); s0 += MAX_SUB) {
+          TcCorrUnit u; memset(&u, 0, sizeof(u));
+          u.cls = (int)ci; u.row0 = r0; u.k0 = k0; u.k1 = k1; u.seg = sg;
+          u.nsub = (int)std::min<size_t>(MAX_SUB, subs.size() - s0);
+          for (int i = 0; i < u.nsub; ++i) { u.det[i] = subs[s0 + i].first; u.col0[i] = subs[s0 + i].second; }
+          cu.push_back(u);
+        }
+      }
   }
-  p->n_ctiles = (int)ct.size();
+  std::stable_sort(cu.begin(), cu.end(), [](const TcCorrUnit &a, const TcCorrUnit &b) {
+    return (long long)a.nsub * (a.k1 - a.k0) > (long long)b.nsub * (b.k1 - b.k0);
+  });
+  p->n_cunits = (int)cu.size();
   // ---- a3: two tensor maps per bank; tiles ordered (bank, template tile, detector, time tile)
   std::vector<TcReconBank> rb(banks.size());
   std::vector<TcReconTile> rt;
@@ -419,15 +497,16 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
         for (int t0 = 0; t0 < B; t0 += TILE_N) rt.push_back({(int)b, det, m0, t0});
   }
   p->n_rtiles = (int)rt.size();
-  if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->ctiles_dev, ct) || !plan_upload(p, &p->rbanks_dev, rb) ||
+  if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   p->recon_grid = std::min(p->n_rtiles, sms);
+  p->corr_grid = std::min(p->n_cunits, sms);
   const int rstages = planes == 2 ? 2 : 4;
   p->recon_smem = rstages * 3 * planes * TILE_BYTES + 1024 + 256;
-  p->corr_smem = 2 * planes * TILE_BYTES + 2 * planes * STRIP_BYTES + 1024 + 256;
+  p->corr_smem = (planes == 2 ? 4 : 6) * planes * TILE_BYTES + 2 * MAX_SUB * planes * STRIP_BYTES + MAX_SUB * XWIN * 4 + 1024 + 256;
   cudaError_t e;
   if (planes == 2) {
     e = cudaFuncSetAttribute(recon_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
@@ -442,9 +521,11 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
 }
 
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
-  if (p->n_ctiles == 0) return cudaSuccess;
-  if (p->planes == 2) corr_tc_kernel<2><<<p->n_ctiles, TC_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->ctiles_dev, n0);
-  else corr_tc_kernel<1><<<p->n_ctiles, TC_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->ctiles_dev, n0);
+  if (p->n_cunits == 0) return cudaSuccess;
+  if (p->planes == 2)
+    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->n_cunits, n0);
+  else
+    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->n_cunits, n0);
   return cudaGetLastError();
 }
 

@@ -105,7 +105,7 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
     b->slices.push_back(std::move(si));
   }
   b->G = (int)b->groups.size();
-  b->Ktot = koff; b->Kpad = (koff + 63) / 64 * 64;
+  b->Ktot = koff; b->Kpad = (koff + 15) / 16 * 16;            // MMA K granularity; TMA zero-fills the rest of a 64-wide box
   if (b->G > LLOID_MAX_GROUPS) { set_error("bank_create: more than %d distinct rates", LLOID_MAX_GROUPS); delete b; return LLOID_EINVAL; }
   // ---- causality: the newest column a push needs, (n0+B)/D + H - 1, must only read
   //      decimated samples that exist, i.e. index <= (n0+B)/D - n_down - 1.

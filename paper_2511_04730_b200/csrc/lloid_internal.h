@@ -38,7 +38,7 @@ struct lloid_bank {
   lloid_options opt;
   std::vector<lloid::SliceInfo> slices;
   std::vector<lloid::GroupInfo> groups;
-  int Ktot, Kpad;                    // sum_s L^s and its round-up to 64
+  int Ktot, Kpad;                    // sum_s L^s and its round-up to 16
   float r_scale;                     // power of two applied to R before the fp16 cast (1 for fp32)
   float *dR32;                       // FFMA:   [2 (re,im)][Mpad][Kpad] fp32
   __half *dR16;                      // tensor: [planes (hi,lo)][2 (re,im)][Mpad][Kpad] fp16, scaled by r_scale
@@ -69,8 +69,10 @@ struct CorrClass {                   // slices (across banks) with identical (ra
   int Lstack, Lpad;                  // stacked basis rows and their round-up to 128
   const float *U32;                  // [Lpad][Npad] fp32 (FFMA path)
   const __half *U16;                 // [planes][Lpad][Npad] fp16 scaled by u_scale (tensor path)
-  float *yring;                      // [n_det][ylen][Lpad] fp32 ring of Y columns; slot of column j = (j + 64) mod ylen
-  long long ydet_stride;
+  float *yring;                      // [nseg][n_det][ylen][Lpad] fp32 ring of Y columns; slot of column j = (j + 64) mod ylen;
+                                     // Y = sum over the nseg tap segments (split-K partial sums, added by the reader in order)
+  long long ydet_stride, yseg_stride;
+  int nseg;
   int ylen, ncols;                   // ncols = B / D new columns per push: [n0/D + H, (n0+B)/D + H)
   float u_scale_inv;
 };
@@ -78,7 +80,7 @@ struct CorrClass {                   // slices (across banks) with identical (ra
 struct CorrTile { int cls, row0, col0; };   // FFMA a2 work item: 64 rows x 64 columns
 
 struct UpItem {                      // one (bank, slice, chunk of <=32 basis rows)
-  const float *yring; long long ydet_stride; int ylen, ypitch, row0, nl;
+  const float *yring; long long ydet_stride, yseg_stride; int nseg, ylen, ypitch, row0, nl;
   int kcol;                          // first column in the bank's Yup (koff_s + chunk*32)
   int g;                             // group of the slice = number of upsample stages
   int log2f[LLOID_MAX_GROUPS];       // log2 f_h of stage h -> h-1, h = 1..g
@@ -109,7 +111,8 @@ cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int
 
 // ---------------------------------------------------------------------------------------------- tcgen05 path (kernels_tc.cu)
 struct TcPlan;
-int tc_time_splits(int B);   // partial peaks per template written by the tensor-core a3 kernel
+int tc_time_splits(int B);
+int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel for a slice of Npad taps   // partial peaks per template written by the tensor-core a3 kernel
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
                    const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes);
 void tc_plan_destroy(TcPlan *p);

@@ -200,8 +200,10 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       }
       __half *p; CK(dev_upload(s, &p, U16)); cc.U16 = p;
     }
-    CK(dev_alloc(s, &cc.yring, (size_t)n_det * cc.ylen * cc.Lpad, true));
+    cc.nseg = (s->precision == LLOID_PREC_FP32_FFMA) ? 1 : tc_k_segments(cc.Npad);
+    CK(dev_alloc(s, &cc.yring, (size_t)cc.nseg * n_det * cc.ylen * cc.Lpad, true));
     cc.ydet_stride = (long long)cc.ylen * cc.Lpad;
+    cc.yseg_stride = (long long)n_det * cc.ydet_stride;
     for (int r0 = 0; r0 < cc.Lstack; r0 += 64)
       for (int c0 = 0; c0 < cc.ncols; c0 += 64) tiles.push_back({(int)c, r0, c0});
     s->work[0] += 2.0 * cc.Lpad * cc.Npad * cc.ncols * n_det;               // executed (padded) flop, one pass
@@ -252,7 +254,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       const CorrClass &cc = s->classes[class_of[Key(si.D, si.N, si.delay, bk->groups[si.group].H)]];
       for (int l0 = 0; l0 < si.L; l0 += 32) {
         UpItem it; memset(&it, 0, sizeof(it));
-        it.yring = cc.yring; it.ydet_stride = cc.ydet_stride; it.ylen = cc.ylen; it.ypitch = cc.Lpad;
+        it.yring = cc.yring; it.ydet_stride = cc.ydet_stride; it.yseg_stride = cc.yseg_stride; it.nseg = cc.nseg; it.ylen = cc.ylen; it.ypitch = cc.Lpad;
         it.row0 = row_off[b][i] + l0; it.nl = std::min(32, si.L - l0); it.kcol = si.koff + l0; it.g = si.group; it.D = si.D;
         for (int h = 1; h <= si.group; ++h) it.log2f[h] = (int)std::lround(std::log2((double)bk->groups[h].f));
         it.yup = yup; it.yup_det_stride = rb.yup_det_stride; it.yup_plane_stride = rb.yup_plane_stride; it.kpitch = bk->Kpad;
