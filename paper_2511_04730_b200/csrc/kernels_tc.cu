@@ -17,7 +17,7 @@
 namespace lloid {
 using namespace ptx;
 
-static constexpr int TC_THREADS = 192;       // 6 warps
+static constexpr int RECON_THREADS = 320;    // a3: warps 0 TMA, 1 MMA, 2-9 epilogue
 static constexpr int TILE_M = 128;           // rows of U / templates of R per tile (= UMMA M, TMEM lanes)
 static constexpr int TILE_N = 128;           // max columns (time samples) per tile
 static constexpr int BK = 64;                // K elements per TMA box = one 128-byte swizzled row of fp16
@@ -42,7 +42,7 @@ struct TcCorrClass {
 //   re += Rre_hi Y_hi (+ Rre_hi Y_lo + Rre_lo Y_hi),  im likewise  -> 2 or 6 MMAs of 128x128x16 per K step.
 // ------------------------------------------------------------------------------------------------
 template <int PLANES>
-__global__ void __launch_bounds__(TC_THREADS, 1)
+__global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, int n_tiles, int n_det, int B,
                 PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank) {
   constexpr int STAGES = PLANES == 2 ? 2 : 4;
@@ -56,7 +56,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 8); }
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -129,42 +129,62 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       }
     }
   } else {
-    // ===== epilogue: thread = one template (TMEM lane), 128 columns in 4 chunks of 32
+    // ===== epilogue (8 warps): thread = one template (TMEM lane) x one half (64 samples) of the tile.  The running
+    // maximum is taken on the raw accumulators (the scale is a power of two, so the order is unchanged).
     const int q = warp & 3;                       // TMEM lane quadrant this warp may access
+    const int half = (warp - 2) >> 2;             // warps 2-5: samples 0-63, warps 6-9: samples 64-127
     int it = 0;
     for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x, ++it) {
       const TcReconTile tl = tiles[ti];
       const TcReconBank *bk = &banks[tl.bank];
       const int buf = it & 1;
+      const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
+      const float sc = bk->inv_scale;
+      const int tbase = tl.t0 + half * (TILE_N / 2);
+      const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < M;
       mbar_wait(&tfull[buf], (it >> 1) & 1);
       tc_fence_after_sync();
-      const int m = tl.m0 + q * 32 + lane;
-      const float sc = bk->inv_scale;
-      const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < bk->M;
-      float *dbg_re = dbg ? snr_debug + ((size_t)tl.det * 2 * bk->M + 2 * m) * B : nullptr;
-      PeakPartial best; best.p = -1.f; best.idx = 0; best.re = 0.f; best.im = 0.f;
-      const uint32_t t_re = tmem + ((uint32_t)(q * 32) << 16) + buf * 256;
+      float bp = -1.f, bre = 0.f, bim = 0.f;
+      int bidx = 0;
+      const uint32_t t_re = tmem + ((uint32_t)(q * 32) << 16) + buf * 256 + half * (TILE_N / 2);
 #pragma unroll 1
-      for (int c = 0; c < TILE_N / 32; ++c) {
+      for (int c = 0; c < TILE_N / 64; ++c) {
         uint32_t vr[32], vi[32];
         tmem_ld_32x32(t_re + c * 32, vr);
         tmem_ld_32x32(t_re + 128 + c * 32, vi);
         tmem_ld_wait();
+        const int t0c = tbase + c * 32;
+        if (t0c + 32 <= B) {
 #pragma unroll
-        for (int i = 0; i < 32; ++i) {
-          const int t = tl.t0 + c * 32 + i;
-          const float re = __uint_as_float(vr[i]) * sc, im = __uint_as_float(vi[i]) * sc;
-          const float p = re * re + im * im;
-          if (t < B) {
-            if (p > best.p) { best.p = p; best.idx = t; best.re = re; best.im = im; }
-            if (dbg) { dbg_re[t] = re; dbg_re[B + t] = im; }
+          for (int i = 0; i < 32; ++i) {
+            const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
+            const float p = fmaf(re, re, im * im);
+            if (p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
           }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 32; ++i) {
+            const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
+            const float p = fmaf(re, re, im * im);
+            if (t0c + i < B && p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
+          }
+        }
+        if (dbg) {
+          float *o = snr_debug + ((size_t)tl.det * 2 * M + 2 * m) * B;
+#pragma unroll
+          for (int i = 0; i < 32; ++i)
+            if (t0c + i < B) { o[t0c + i] = __uint_as_float(vr[i]) * sc; o[B + t0c + i] = __uint_as_float(vi[i]) * sc; }
         }
       }
       tc_fence_before_sync();
       __syncwarp();
       if (lane == 0) mbar_arrive(&tempty[buf]);
-      if (m < bk->M) partial[((size_t)tl.det * Mtot + bk->tmpl_off + m) * n_tt + tl.t0 / TILE_N] = best;
+      if (m < M) {
+        PeakPartial best;
+        best.re = bre * sc; best.im = bim * sc; best.idx = bidx;
+        best.p = (bp < 0.f) ? -1.f : best.re * best.re + best.im * best.im;
+        partial[((size_t)tl.det * Mtot + tmpl_off + m) * n_tt + (tl.t0 / TILE_N) * 2 + half] = best;
+      }
     }
   }
   tc_fence_before_sync();
@@ -395,7 +415,7 @@ struct TcPlan {
   std::vector<void *> allocs;
 };
 
-int tc_time_splits(int B) { return (B + TILE_N - 1) / TILE_N; }
+int tc_time_splits(int B) { return 2 * ((B + TILE_N - 1) / TILE_N); }   // two 64-sample halves per tile
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -531,10 +551,10 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
   if (p->planes == 2)
-    recon_tc_kernel<2><<<p->recon_grid, TC_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
+    recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
                                                                          partial, Mtot, p->n_tt, snr_debug, debug_bank);
   else
-    recon_tc_kernel<1><<<p->recon_grid, TC_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
+    recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
                                                                          partial, Mtot, p->n_tt, snr_debug, debug_bank);
   return cudaGetLastError();
 }
