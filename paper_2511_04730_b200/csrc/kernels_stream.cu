@@ -296,19 +296,35 @@ cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int
 // (strict '>' keeps the first maximum), then snr = sqrt(p), phase = atan2(im, re).
 // The last thread also advances the device-side stream clock n0 by B.
 // ------------------------------------------------------------------------------------------------
-__global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_det, int Mtot, int n_tt,
+__global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_det, int Mtot, int n_tt, int g,
                                 float threshold, lloid_peak *__restrict__ peaks, long long *n0, int B) {
-  int t = blockIdx.x * blockDim.x + threadIdx.x;
-  if (t == 0) *n0 += B;
-  if (t >= n_det * Mtot) return;
-  const PeakPartial *pp = partial + (size_t)t * n_tt;
-  PeakPartial best = pp[0];
-  for (int i = 1; i < n_tt; ++i) {
-    PeakPartial c = pp[i];
-    if (c.p > best.p) best = c;
+  // g (power of two <= 32) consecutive lanes share one template: coalesced reads of its n_tt partial peaks, then a
+  // shuffle reduction.  "Better" = larger |z|^2, ties -> lower sample index (= the first maximum in time).
+  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (gt == 0) *n0 += B;
+  const long long t = gt / g;
+  const int li = (int)(gt % g);
+  const bool valid = t < (long long)n_det * Mtot;
+  PeakPartial best;
+  best.p = -2.f; best.idx = 0x7fffffff; best.re = 0.f; best.im = 0.f;
+  if (valid) {
+    const PeakPartial *pp = partial + (size_t)t * n_tt;
+    for (int i = li; i < n_tt; i += g) {
+      PeakPartial c = pp[i];
+      if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
+    }
   }
+  for (int o = g >> 1; o > 0; o >>= 1) {
+    PeakPartial c;
+    c.p = __shfl_xor_sync(0xffffffffu, best.p, o);
+    c.idx = __shfl_xor_sync(0xffffffffu, best.idx, o);
+    c.re = __shfl_xor_sync(0xffffffffu, best.re, o);
+    c.im = __shfl_xor_sync(0xffffffffu, best.im, o);
+    if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
+  }
+  if (!valid || li != 0) return;
   lloid_peak o;
-  o.snr = sqrtf(best.p);
+  o.snr = sqrtf(fmaxf(best.p, 0.f));
   o.sample = best.idx;
   o.phase = atan2f(best.im, best.re);
   if (threshold > 0.f && o.snr < threshold) { o.snr = 0.f; o.sample = -1; o.phase = 0.f; }
@@ -317,8 +333,10 @@ __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_d
 
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
                             lloid_peak *peaks, long long *n0, int B, cudaStream_t st) {
-  int n = n_det * Mtot;
-  finalize_kernel<<<(n + 255) / 256, 256, 0, st>>>(partial, n_det, Mtot, n_tt, threshold, peaks, n0, B);
+  int g = 1;
+  while (g < n_tt && g < 32) g <<= 1;
+  const long long n = (long long)n_det * Mtot * g;
+  finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partial, n_det, Mtot, n_tt, g, threshold, peaks, n0, B);
   return cudaGetLastError();
 }
 

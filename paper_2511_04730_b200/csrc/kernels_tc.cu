@@ -23,7 +23,7 @@ static constexpr int TILE_N = 128;           // max columns (time samples) per t
 static constexpr int BK = 64;                // K elements per TMA box = one 128-byte swizzled row of fp16
 static constexpr int TILE_BYTES = TILE_M * BK * 2;   // 16 KB
 
-struct TcReconTile { int bank, det, m0, t0; };
+struct TcReconTile { int bank, det, m0, t0, nt, slot; };   // nt consecutive time tiles starting at sample t0; partial slot
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
   CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 64 x 128
   CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 64 x 128
@@ -73,6 +73,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         const TcReconTile tl = tiles[ti];
         const TcReconBank *bk = &banks[tl.bank];
         const int nkb = (bk->Kpad + BK - 1) / BK;
+        for (int tt = 0; tt < tl.nt; ++tt)
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(&empty[stage], phase ^ 1);
           mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
@@ -81,7 +82,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           for (int p = 0; p < PLANES; ++p) {
             tma_load_2d(s + (3 * p + 0) * TILE_BYTES, &bk->mapR, &full[stage], kb * BK, (p * 2 + 0) * bk->Mpad + tl.m0);
             tma_load_2d(s + (3 * p + 1) * TILE_BYTES, &bk->mapR, &full[stage], kb * BK, (p * 2 + 1) * bk->Mpad + tl.m0);
-            tma_load_2d(s + (3 * p + 2) * TILE_BYTES, &bk->mapY, &full[stage], kb * BK, (p * n_det + tl.det) * B + tl.t0);
+            tma_load_2d(s + (3 * p + 2) * TILE_BYTES, &bk->mapY, &full[stage], kb * BK, (p * n_det + tl.det) * B + tl.t0 + tt * TILE_N);
           }
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
@@ -92,9 +93,10 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     if (lane == 0) {
       constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N);
       int stage = 0; uint32_t phase = 0; int it = 0;
-      for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x, ++it) {
+      for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
         const TcReconTile tl = tiles[ti];
         const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
+        for (int tt = 0; tt < tl.nt; ++tt, ++it) {
         const int buf = it & 1;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
@@ -126,6 +128,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
         mma_commit(&tfull[buf]);
+        }
       }
     }
   } else {
@@ -134,56 +137,58 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     const int q = warp & 3;                       // TMEM lane quadrant this warp may access
     const int half = (warp - 2) >> 2;             // warps 2-5: samples 0-63, warps 6-9: samples 64-127
     int it = 0;
-    for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x, ++it) {
+    for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
       const TcReconTile tl = tiles[ti];
       const TcReconBank *bk = &banks[tl.bank];
-      const int buf = it & 1;
       const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
       const float sc = bk->inv_scale;
-      const int tbase = tl.t0 + half * (TILE_N / 2);
       const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < M;
-      mbar_wait(&tfull[buf], (it >> 1) & 1);
-      tc_fence_after_sync();
-      float bp = -1.f, bre = 0.f, bim = 0.f;
+      float bp = -1.f, bre = 0.f, bim = 0.f;      // running first maximum over the unit's nt tiles (ascending time)
       int bidx = 0;
-      const uint32_t t_re = tmem + ((uint32_t)(q * 32) << 16) + buf * 256 + half * (TILE_N / 2);
+      for (int tt = 0; tt < tl.nt; ++tt, ++it) {
+        const int buf = it & 1;
+        const int tbase = tl.t0 + tt * TILE_N + half * (TILE_N / 2);
+        mbar_wait(&tfull[buf], (it >> 1) & 1);
+        tc_fence_after_sync();
+        const uint32_t t_re = tmem + ((uint32_t)(q * 32) << 16) + buf * 256 + half * (TILE_N / 2);
 #pragma unroll 1
-      for (int c = 0; c < TILE_N / 64; ++c) {
-        uint32_t vr[32], vi[32];
-        tmem_ld_32x32(t_re + c * 32, vr);
-        tmem_ld_32x32(t_re + 128 + c * 32, vi);
-        tmem_ld_wait();
-        const int t0c = tbase + c * 32;
-        if (t0c + 32 <= B) {
+        for (int c = 0; c < TILE_N / 64; ++c) {
+          uint32_t vr[32], vi[32];
+          tmem_ld_32x32(t_re + c * 32, vr);
+          tmem_ld_32x32(t_re + 128 + c * 32, vi);
+          tmem_ld_wait();
+          const int t0c = tbase + c * 32;
+          if (t0c + 32 <= B) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
-            const float p = fmaf(re, re, im * im);
-            if (p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
+            for (int i = 0; i < 32; ++i) {
+              const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
+              const float p = fmaf(re, re, im * im);
+              if (p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
+            }
+          } else {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
+              const float p = fmaf(re, re, im * im);
+              if (t0c + i < B && p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
+            }
           }
-        } else {
+          if (dbg) {
+            float *o = snr_debug + ((size_t)tl.det * 2 * M + 2 * m) * B;
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
-            const float p = fmaf(re, re, im * im);
-            if (t0c + i < B && p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
+            for (int i = 0; i < 32; ++i)
+              if (t0c + i < B) { o[t0c + i] = __uint_as_float(vr[i]) * sc; o[B + t0c + i] = __uint_as_float(vi[i]) * sc; }
           }
         }
-        if (dbg) {
-          float *o = snr_debug + ((size_t)tl.det * 2 * M + 2 * m) * B;
-#pragma unroll
-          for (int i = 0; i < 32; ++i)
-            if (t0c + i < B) { o[t0c + i] = __uint_as_float(vr[i]) * sc; o[B + t0c + i] = __uint_as_float(vi[i]) * sc; }
-        }
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[buf]);
       }
-      tc_fence_before_sync();
-      __syncwarp();
-      if (lane == 0) mbar_arrive(&tempty[buf]);
       if (m < M) {
         PeakPartial best;
         best.re = bre * sc; best.im = bim * sc; best.idx = bidx;
         best.p = (bp < 0.f) ? -1.f : best.re * best.re + best.im * best.im;
-        partial[((size_t)tl.det * Mtot + tmpl_off + m) * n_tt + (tl.t0 / TILE_N) * 2 + half] = best;
+        partial[((size_t)tl.det * Mtot + tmpl_off + m) * n_tt + tl.slot * 2 + half] = best;
       }
     }
   }
@@ -415,7 +420,18 @@ struct TcPlan {
   std::vector<void *> allocs;
 };
 
-int tc_time_splits(int B) { return 2 * ((B + TILE_N - 1) / TILE_N); }   // two 64-sample halves per tile
+// Consecutive time tiles one CTA visit covers for a fixed (bank, detector, template tile): as long as possible while
+// the persistent grid still gets >= 3 units per SM.  The peak is carried in registers across the run.
+static int recon_run_tiles(int B, long long n_mtile_units) {
+  const int ntile = (B + TILE_N - 1) / TILE_N;
+  int nt = 1;
+  while (nt * 2 <= ntile && n_mtile_units * ((ntile + 2 * nt - 1) / (2 * nt)) >= 3 * 148) nt *= 2;
+  return nt;
+}
+int tc_time_splits(int B, long long n_mtile_units) {          // partial peaks per template: 2 halves per run
+  const int ntile = (B + TILE_N - 1) / TILE_N, nt = recon_run_tiles(B, n_mtile_units);
+  return 2 * ((ntile + nt - 1) / nt);
+}
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
                                   const cuuint32_t *, const cuuint32_t *, CUtensorMapInterleave, CUtensorMapSwizzle,
@@ -472,7 +488,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
                    const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes) {
   *out = nullptr;
   TcPlan *p = new TcPlan();
-  p->planes = planes; p->n_det = n_det; p->B = B; p->n_tt = tc_time_splits(B); p->classes_dev = classes_dev;
+  p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
   // ---- a2: one tensor map per class; units = (row tile, tap segment, group of <= 4 (detector, column tile) sub-tiles),
   //      dealt to the persistent CTAs in order of decreasing cost
   std::vector<TcCorrClass> cm(classes.size());
@@ -512,9 +528,16 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad) ||
         !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
+  }
+  long long n_mu = 0;
+  for (const ReconBank &k : banks) n_mu += (long long)((k.M + TILE_M - 1) / TILE_M) * n_det;
+  const int nt = recon_run_tiles(B, n_mu), ntile = (B + TILE_N - 1) / TILE_N;
+  p->n_tt = tc_time_splits(B, n_mu);
+  for (size_t b = 0; b < banks.size(); ++b) {
+    const ReconBank &k = banks[b];
     for (int m0 = 0; m0 < k.M; m0 += TILE_M)
       for (int det = 0; det < n_det; ++det)
-        for (int t0 = 0; t0 < B; t0 += TILE_N) rt.push_back({(int)b, det, m0, t0});
+        for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
   }
   p->n_rtiles = (int)rt.size();
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||

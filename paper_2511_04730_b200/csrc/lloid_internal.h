@@ -111,7 +111,7 @@ cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int
 
 // ---------------------------------------------------------------------------------------------- tcgen05 path (kernels_tc.cu)
 struct TcPlan;
-int tc_time_splits(int B);
+int tc_time_splits(int B, long long n_mtile_units);   // n_mtile_units = sum_banks ceil(M/128) * n_det
 int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel for a slice of Npad taps   // partial peaks per template written by the tensor-core a3 kernel
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
                    const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes);

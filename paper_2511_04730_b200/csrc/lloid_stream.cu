@@ -272,7 +272,9 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->n_items = (int)items.size();
   CK(dev_upload(s, &s->items_dev, items));
   CK(dev_upload(s, &s->rbanks_dev, s->rbanks));
-  s->n_tt = (s->precision == LLOID_PREC_FP32_FFMA) ? (B + 63) / 64 : tc_time_splits(B);
+  long long n_mu = 0;
+  for (const lloid_bank *bk : s->banks) n_mu += (long long)((bk->M + 127) / 128) * n_det;
+  s->n_tt = (s->precision == LLOID_PREC_FP32_FFMA) ? (B + 63) / 64 : tc_time_splits(B, n_mu);
   CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
