@@ -103,7 +103,8 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   slices becomes one contraction over the concatenated basis axis at f0.
 //   Stage h -> h-1 with factor f:  out[i] = in[i/f] if i mod f == 0 (Eq. 8 case 1), else
 //   sum_{k=0}^{15} in[floor(i/f) + 8 - k] * g_f[k f + (i mod f)]   (Eq. 7-8, zero-phase form).
-//   CTA = (time chunk of `chunk` f0 samples, item = 32 basis rows of one slice, detector).  lane = basis row.
+//   CTA = (time chunk of `chunk` f0 samples, item = 32 basis rows sharing one upsample chain, detector).
+//   lane = basis row (of any slice / bank with that chain: UpRow gives its source ring row and destination column).
 // ------------------------------------------------------------------------------------------------
 #define UP_RUN 8
 struct UpTaps2 { float t[16]; };   // g_2[2k+1], k = 0..15: the 16 non-zero taps of the x2 interpolation phase (Eq. 7)
@@ -120,7 +121,7 @@ __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_strid
 }
 
 template <int HALF_PLANES>
-__global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restrict__ items, int B, int chunk,
+__global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
                                                           const float *__restrict__ uptaps,
                                                           const int *__restrict__ uptap_off,
                                                           const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
@@ -150,18 +151,19 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   }
   __syncthreads();
   const bool active = lane < it->nl;
-  const int ylen = it->ylen, ypitch = it->ypitch, kpitch = it->kpitch;
-  const float *yr = it->yring + (size_t)det * it->ydet_stride + it->row0 + lane;
-  const int nseg = it->nseg;
-  const size_t yseg = (size_t)it->yseg_stride;
+  const UpRow *rw = &rows[it->row0 + (active ? lane : 0)];     // this lane's row: source ring row and destination column
+  const int ylen = it->ylen, ypitch = rw->ypitch, kpitch = rw->kpitch;
+  const float *yr = rw->ysrc + (size_t)det * rw->ydet_stride;
+  const int nseg = rw->nseg;
+  const size_t yseg = (size_t)rw->yseg_stride;
   auto load_y = [&](int sl) {                              // split-K partial sums added in segment order
     float v = yr[(size_t)sl * ypitch];
     for (int sg = 1; sg < nseg; ++sg) v += yr[sg * yseg + (size_t)sl * ypitch];
     return v;
   };
-  void *yup = it->yup;
-  const size_t plane_stride = (size_t)it->yup_plane_stride;
-  const size_t out0 = (size_t)det * it->yup_det_stride + (size_t)it->kcol + lane + (size_t)ka * kpitch;   // sample ka
+  void *yup = rw->yup;
+  const size_t plane_stride = (size_t)rw->yup_plane_stride;
+  const size_t out0 = (size_t)det * rw->yup_det_stride + (size_t)rw->dst0 + (size_t)ka * kpitch;   // sample ka
 
   // level G from the Y ring (columns never computed at stream start are the ring's zeros)
   const int wg = s_w[G];
@@ -273,7 +275,7 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   }
 }
 
-cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
+cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
                             const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
   static UpTaps2 t2;                                     // Eq. 4 with f = 2, c = 16 (same float64 -> fp32 values as uptaps)
@@ -285,9 +287,9 @@ cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int
     }
     have = true;
   }
-  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else upsample_kernel<2><<<grid, 256, 0, st>>>(items_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else upsample_kernel<2><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   return cudaGetLastError();
 }
 

@@ -79,13 +79,19 @@ struct CorrClass {                   // slices (across banks) with identical (ra
 
 struct CorrTile { int cls, row0, col0; };   // FFMA a2 work item: 64 rows x 64 columns
 
-struct UpItem {                      // one (bank, slice, chunk of <=32 basis rows)
-  const float *yring; long long ydet_stride, yseg_stride; int nseg, ylen, ypitch, row0, nl;
-  int kcol;                          // first column in the bank's Yup (koff_s + chunk*32)
-  int g;                             // group of the slice = number of upsample stages
+struct UpRow {                       // one basis row of one slice of one bank: where it comes from and where it goes
+  const float *ysrc;                 // class Y ring + stacked row index (detector 0, segment 0)
+  long long ydet_stride, yseg_stride;
+  void *yup;                         // bank's upsampled-Y array (plane 0)
+  long long dst0;                    // element offset of (detector 0, sample 0, this row's column)
+  long long yup_det_stride, yup_plane_stride;
+  int nseg, ypitch, kpitch, pad_;
+};
+struct UpItem {                      // <= 32 rows (lanes) that share one upsample chain: (rate, stage factors)
+  int row0, nl;                      // rows [row0, row0 + nl) of the UpRow table
+  int g;                             // number of upsample stages
   int log2f[LLOID_MAX_GROUPS];       // log2 f_h of stage h -> h-1, h = 1..g
-  int D;                             // D of the slice's group
-  void *yup; long long yup_det_stride, yup_plane_stride; int kpitch;
+  int ylen;                          // Y ring length at this rate (B/D + 32)
 };
 
 struct ReconBank {                   // a3 work description of one bank
@@ -102,7 +108,7 @@ struct PeakPartial { float p; int idx; float re, im; };
 cudaError_t launch_decimate(const DecimParams &P, const float *strain, const long long *n0, cudaStream_t st);
 cudaError_t launch_corr_ffma(const CorrClass *cls_dev, const CorrTile *tiles_dev, int n_tiles, int n_det,
                              const long long *n0, cudaStream_t st);
-cudaError_t launch_upsample(const UpItem *items_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
+cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
                             const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st);
 cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);

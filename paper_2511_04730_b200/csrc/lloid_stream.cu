@@ -23,7 +23,7 @@ struct lloid_stream {
   std::vector<CorrClass> classes;
   CorrClass *classes_dev;
   CorrTile *tiles_dev; int n_tiles;
-  UpItem *items_dev; int n_items;
+  UpItem *items_dev; UpRow *uprows_dev; int n_items;
   float *uptaps_dev; int *uptap_off_dev;
   ReconBank *rbanks_dev;
   std::vector<ReconBank> rbanks;
@@ -230,7 +230,9 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   }
 
   // ---- per-bank Yup buffers, upsample items, reconstruction descriptors
-  std::vector<UpItem> items;
+  // rows are grouped by upsample chain (stage factors) so that a warp's 32 lanes are 32 rows of ANY slices / banks
+  // sharing the chain; within a chain they are ordered by (bank, column) to keep the stores contiguous
+  std::map<std::vector<int>, std::vector<UpRow>> chains;
   s->Mtot = 0; s->max_mtiles = 0;
   for (int b = 0; b < n_banks; ++b) {
     const lloid_bank *bk = s->banks[b];
@@ -252,13 +254,17 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     for (int i = 0; i < bk->S; ++i) {
       const SliceInfo &si = bk->slices[i];
       const CorrClass &cc = s->classes[class_of[Key(si.D, si.N, si.delay, bk->groups[si.group].H)]];
-      for (int l0 = 0; l0 < si.L; l0 += 32) {
-        UpItem it; memset(&it, 0, sizeof(it));
-        it.yring = cc.yring; it.ydet_stride = cc.ydet_stride; it.yseg_stride = cc.yseg_stride; it.nseg = cc.nseg; it.ylen = cc.ylen; it.ypitch = cc.Lpad;
-        it.row0 = row_off[b][i] + l0; it.nl = std::min(32, si.L - l0); it.kcol = si.koff + l0; it.g = si.group; it.D = si.D;
-        for (int h = 1; h <= si.group; ++h) it.log2f[h] = (int)std::lround(std::log2((double)bk->groups[h].f));
-        it.yup = yup; it.yup_det_stride = rb.yup_det_stride; it.yup_plane_stride = rb.yup_plane_stride; it.kpitch = bk->Kpad;
-        items.push_back(it);
+      std::vector<int> key;
+      key.push_back(si.D);
+      for (int h = 1; h <= si.group; ++h) key.push_back((int)std::lround(std::log2((double)bk->groups[h].f)));
+      std::vector<UpRow> &dst = chains[key];
+      for (int l = 0; l < si.L; ++l) {
+        UpRow r; memset(&r, 0, sizeof(r));
+        r.ysrc = cc.yring + row_off[b][i] + l; r.ydet_stride = cc.ydet_stride; r.yseg_stride = cc.yseg_stride;
+        r.nseg = cc.nseg; r.ypitch = cc.Lpad;
+        r.yup = yup; r.dst0 = si.koff + l; r.yup_det_stride = rb.yup_det_stride; r.yup_plane_stride = rb.yup_plane_stride;
+        r.kpitch = bk->Kpad;
+        dst.push_back(r);
       }
       rate_sum += (double)si.L * si.rate;
     }
@@ -269,8 +275,22 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     s->work[5] += 2.0 * bk->Mpad * bk->Kpad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
     s->work[6] += 2.0 * plane_elems * (s->up_planes == 0 ? 4 : 2 * planes);
   }
+  std::vector<UpItem> items;
+  std::vector<UpRow> uprows;
+  for (auto &kv : chains) {
+    const std::vector<int> &key = kv.first;
+    for (size_t r0 = 0; r0 < kv.second.size(); r0 += 32) {
+      UpItem it; memset(&it, 0, sizeof(it));
+      it.row0 = (int)(uprows.size() + r0); it.nl = (int)std::min<size_t>(32, kv.second.size() - r0);
+      it.g = (int)key.size() - 1; it.ylen = B / key[0] + 32;
+      for (int h = 1; h <= it.g; ++h) it.log2f[h] = key[h];
+      items.push_back(it);
+    }
+    uprows.insert(uprows.end(), kv.second.begin(), kv.second.end());
+  }
   s->n_items = (int)items.size();
   CK(dev_upload(s, &s->items_dev, items));
+  CK(dev_upload(s, &s->uprows_dev, uprows));
   CK(dev_upload(s, &s->rbanks_dev, s->rbanks));
   long long n_mu = 0;
   for (const lloid_bank *bk : s->banks) n_mu += (long long)((bk->M + 127) / 128) * n_det;
@@ -313,7 +333,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   }
   mark(2);
   if (e == cudaSuccess)
-    e = launch_upsample(s->items_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
+    e = launch_upsample(s->items_dev, s->uprows_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
                         s->n0_dev, s->up_planes, s->st);
   mark(3);
   if (e == cudaSuccess) {
