@@ -127,3 +127,63 @@ def test_multirate_bank_two_detectors(precision):
         print(f"multirate det {det}: max err {emax:.3e} rms {erms:.3e}")
         assert emax <= TOL[precision]
         check_peaks(peaks[:, det, :], rho_ref, B, TOL[precision] * 2 * np.sqrt(2.0))
+
+
+def test_ragged_buffer_threshold_and_host_push():
+    """Buffer length that is not a multiple of the 128-sample tile (B = 320), a ragged template count, the threshold
+    option, and lloid_stream_push_host (host buffers, copies inside the call) against the device-pointer push."""
+    _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import find_peaks, lloid_snr
+    from workloads import make_strain, random_bank
+    bank = random_bank(21, 70, [(2048, 512, 17), (1024, 768, 33), (512, 640, 21), (512, 384, 9)]).as_f32()
+    B, n_push = 320, 6
+    strain = np.stack([make_strain(210 + d, B * n_push) for d in range(2)])
+    strain[0, 4 * B + 100] += 30.0                      # a glitch: some templates ring above threshold in push 4
+    for precision in (2, 0):
+        rho_gpu, peaks = run_gpu([bank], strain, B, precision)
+        thr = 4.0                                        # PAPER.md:199 trigger threshold
+        st = lib.LloidStream([bank], 2, B, precision=precision, threshold=thr)
+        for p in range(n_push):
+            st.strain_host.copy_(st.torch.from_numpy(strain[:, p * B:(p + 1) * B].copy()))
+            pk_host = st.push_host().copy()
+            ref_pk = peaks[p]
+            above = ref_pk["snr"] >= thr
+            assert np.array_equal(pk_host["sample"][above], ref_pk["sample"][above])
+            assert np.array_equal(pk_host["snr"][above], ref_pk["snr"][above])          # same kernels: bit-identical
+            assert (pk_host["sample"][~above] == -1).all() and (pk_host["snr"][~above] == 0).all()
+        st.close()
+        for det in range(2):
+            ref = lloid_snr(bank, strain[det])
+            emax, _ = check_snr(rho_gpu[det], ref, TOL[precision])
+            assert emax <= TOL[precision]
+            check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0) * 3)
+        assert (peaks["snr"][4, 0] >= thr).any()
+
+
+def test_two_streams_share_banks_and_errors():
+    """Two streams over the same bank handles keep independent state; debug_bank out of range -> LLOID_ESTATE."""
+    _torch_cuda()
+    import torch
+    import paper_2511_04730_b200 as lib
+    from workloads import make_strain, random_bank
+    bank = random_bank(5, 33, [(2048, 256, 12), (1024, 384, 20)]).as_f32()
+    h = lib.lloid_bank_create(bank.f0, bank.M, lib.bank_slices(bank), lib.LLOID_PREC_F16_SPLIT)
+    s1 = lib.lloid_stream_create([h], 1, 512)
+    s2 = lib.lloid_stream_create([h], 1, 512)
+    x = torch.from_numpy(np.stack([make_strain(9, 1024)])).cuda()
+    pk = torch.zeros((3, 1, 33, 3), dtype=torch.int32, device="cuda")
+    lib.lloid_stream_push(s1, x[:, :512].contiguous().data_ptr(), pk[0].data_ptr())
+    lib.lloid_stream_push(s1, x[:, 512:].contiguous().data_ptr(), pk[1].data_ptr())
+    lib.lloid_stream_push(s2, x[:, :512].contiguous().data_ptr(), pk[2].data_ptr())     # s2 starts at sample 0
+    torch.cuda.synchronize()
+    assert torch.equal(pk[0], pk[2]) and not torch.equal(pk[1], pk[2])
+    assert lib.lloid_stream_samples_pushed(s1) == 1024 and lib.lloid_stream_samples_pushed(s2) == 512
+    snr = torch.zeros((1, 66, 512), device="cuda")
+    with pytest.raises(lib.LloidError) as e:
+        lib.lloid_stream_push(s1, x[:, :512].contiguous().data_ptr(), pk[0].data_ptr(), snr.data_ptr(), 3)
+    assert e.value.code == lib.LLOID_ESTATE
+    with pytest.raises(lib.LloidError) as e:
+        lib.lloid_stream_create([h], 1, 101)            # not a multiple of the largest decimation factor (2)
+    assert e.value.code == lib.LLOID_EINVAL
+    lib.lloid_stream_destroy(s1); lib.lloid_stream_destroy(s2); lib.lloid_bank_destroy(h)
