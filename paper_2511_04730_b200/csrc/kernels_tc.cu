@@ -10,6 +10,7 @@
 
 #include <algorithm>
 #include <cstring>
+#include <queue>
 
 #include "lloid_internal.h"
 #include "tc_ptx.cuh"
@@ -43,7 +44,8 @@ struct TcCorrClass {
 // ------------------------------------------------------------------------------------------------
 template <int PLANES>
 __global__ void __launch_bounds__(RECON_THREADS, 1)
-recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, int n_tiles, int n_det, int B,
+recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
+                int n_det, int B,
                 PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank) {
   constexpr int STAGES = PLANES == 2 ? 2 : 4;
   constexpr int STAGE_BYTES = 3 * PLANES * TILE_BYTES;        // Rre, Rim, Y per plane
@@ -69,7 +71,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     // ===== TMA producer
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
+      for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
         const TcReconTile tl = tiles[ti];
         const TcReconBank *bk = &banks[tl.bank];
         const int nkb = (bk->Kpad + BK - 1) / BK;
@@ -93,7 +95,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     if (lane == 0) {
       constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N);
       int stage = 0; uint32_t phase = 0; int it = 0;
-      for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
+      for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
         const TcReconTile tl = tiles[ti];
         const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
         for (int tt = 0; tt < tl.nt; ++tt, ++it) {
@@ -137,7 +139,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     const int q = warp & 3;                       // TMEM lane quadrant this warp may access
     const int half = (warp - 2) >> 2;             // warps 2-5: samples 0-63, warps 6-9: samples 64-127
     int it = 0;
-    for (int ti = blockIdx.x; ti < n_tiles; ti += gridDim.x) {
+    for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
       const TcReconTile tl = tiles[ti];
       const TcReconBank *bk = &banks[tl.bank];
       const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
@@ -225,7 +227,7 @@ int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
 template <int PLANES>
 __global__ void __launch_bounds__(CORR_THREADS, 1)
 corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restrict__ maps, const TcCorrUnit *__restrict__ units,
-               int n_units, const long long *__restrict__ n0_ptr) {
+               const int *__restrict__ cta_begin, const long long *__restrict__ n0_ptr) {
   constexpr int STAGES = PLANES == 2 ? 4 : 6;
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -253,7 +255,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
     // ===== TMA producer: U tiles of 128 rows x 64 taps (x planes), in unit order
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x) {
+      for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui) {
         const TcCorrUnit *u = &units[ui];
         const CUtensorMap *mapU = &maps[u->cls].mapU;
         const int Lpad = classes[u->cls].Lpad, row0 = u->row0, k1 = u->k1;
@@ -271,7 +273,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
     // ===== MMA issuer.  Descriptors differ only in their 14-bit address field (16-byte units): one 64-bit add each.
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0; int it = 0, chunk_it = 0;
-      for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x, ++it) {
+      for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
         const TcCorrUnit *u = &units[ui];
         const int nsub = u->nsub, ncols = classes[u->cls].ncols, k0 = u->k0, k1 = u->k1;
         const uint32_t idesc0 = idesc_f16_f32(TILE_M, min(TILE_N, (ncols - u->col0[0] + 15) & ~15));
@@ -317,7 +319,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
     const int tid = threadIdx.x - 192;
     const long long n0 = *n0_ptr;
     int chunk_it = 0;
-    for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x) {
+    for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui) {
       const TcCorrUnit *u = &units[ui];
       const CorrClass &c = classes[u->cls];
       const int nsub = u->nsub, k0 = u->k0, klen = u->k1 - k0;
@@ -372,7 +374,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
     const int q = warp & 3;
     const long long n0 = *n0_ptr;
     int it = 0;
-    for (int ui = blockIdx.x; ui < n_units; ui += gridDim.x, ++it) {
+    for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
       const TcCorrUnit *u = &units[ui];
       const CorrClass &c = classes[u->cls];
       const int nsub = u->nsub, buf = it & 1;
@@ -414,6 +416,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 struct TcPlan {
   int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
+  int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
   int recon_grid, recon_smem, corr_smem;
@@ -431,6 +434,35 @@ static int recon_run_tiles(int B, long long n_mtile_units) {
 int tc_time_splits(int B, long long n_mtile_units) {          // partial peaks per template: 2 halves per run
   const int ntile = (B + TILE_N - 1) / TILE_N, nt = recon_run_tiles(B, n_mtile_units);
   return 2 * ((ntile + nt - 1) / nt);
+}
+
+// Longest-processing-time assignment of work items to `grid` persistent CTAs: items sorted by decreasing cost, each given
+// to the least loaded CTA; returns the items regrouped per CTA and the per-CTA begin offsets.
+template <typename T, typename CostFn>
+static void lpt_assign(std::vector<T> &items, int grid, CostFn cost, std::vector<int> &begin) {
+  std::vector<int> order(items.size());
+  for (size_t i = 0; i < order.size(); ++i) order[i] = (int)i;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) { return cost(items[a]) > cost(items[b]); });
+  std::vector<long long> load(grid, 0);
+  std::vector<std::vector<int>> mine(grid);
+  typedef std::pair<long long, int> Q;
+  std::priority_queue<Q, std::vector<Q>, std::greater<Q>> heap;
+  for (int c = 0; c < grid; ++c) heap.push({0, c});
+  for (int i : order) {
+    Q q = heap.top(); heap.pop();
+    mine[q.second].push_back(i);
+    q.first += cost(items[i]);
+    heap.push(q);
+  }
+  std::vector<T> out;
+  out.reserve(items.size());
+  begin.assign(grid + 1, 0);
+  for (int c = 0; c < grid; ++c) {
+    begin[c] = (int)out.size();
+    for (int i : mine[c]) out.push_back(items[i]);
+  }
+  begin[grid] = (int)out.size();
+  items.swap(out);
 }
 
 typedef CUresult (*EncodeTiledFn)(CUtensorMap *, CUtensorMapDataType, cuuint32_t, void *, const cuuint64_t *, const cuuint64_t *,
@@ -515,9 +547,6 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
         }
       }
   }
-  std::stable_sort(cu.begin(), cu.end(), [](const TcCorrUnit &a, const TcCorrUnit &b) {
-    return (long long)a.nsub * (a.k1 - a.k0) > (long long)b.nsub * (b.k1 - b.k0);
-  });
   p->n_cunits = (int)cu.size();
   // ---- a3: two tensor maps per bank; tiles ordered (bank, template tile, detector, time tile)
   std::vector<TcReconBank> rb(banks.size());
@@ -540,13 +569,17 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
         for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
   }
   p->n_rtiles = (int)rt.size();
-  if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
-      !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
-  p->recon_grid = std::min(p->n_rtiles, sms);
-  p->corr_grid = std::min(p->n_cunits, sms);
+  p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
+  p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
+  std::vector<int> cbegin, rbegin;
+  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)u.nsub * (u.k1 - u.k0) + 128; }, cbegin);
+  lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * ((rb[t.bank].Kpad + BK - 1) / BK + 1); }, rbegin);
+  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+  if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
+      !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   const int rstages = planes == 2 ? 2 : 4;
   p->recon_smem = rstages * 3 * planes * TILE_BYTES + 1024 + 256;
   p->corr_smem = (planes == 2 ? 4 : 6) * planes * TILE_BYTES + 2 * MAX_SUB * planes * STRIP_BYTES + MAX_SUB * XWIN * 4 + 1024 + 256;
@@ -566,18 +599,18 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
   if (p->n_cunits == 0) return cudaSuccess;
   if (p->planes == 2)
-    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->n_cunits, n0);
+    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
   else
-    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->n_cunits, n0);
+    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
   return cudaGetLastError();
 }
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
   if (p->planes == 2)
-    recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
+    recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
                                                                          partial, Mtot, p->n_tt, snr_debug, debug_bank);
   else
-    recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->n_rtiles, p->n_det, p->B,
+    recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
                                                                          partial, Mtot, p->n_tt, snr_debug, debug_bank);
   return cudaGetLastError();
 }
