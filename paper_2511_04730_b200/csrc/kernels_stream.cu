@@ -14,6 +14,7 @@ namespace lloid {
 //   DEC_PER_CTA outputs per CTA; thread t sums taps t, t+256, ... then a fixed-order reduction: deterministic.
 // ------------------------------------------------------------------------------------------------
 #define DEC_PER_CTA 8
+#define DEC_WIN (2 * 32 * 64 + 1 + (DEC_PER_CTA - 1) * 64 + 3)   // staged strain span: n_down = 32, D <= 64
 __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, const float *__restrict__ strain,
                                                        const long long *__restrict__ n0_ptr) {
   const long long n0 = *n0_ptr;
@@ -50,24 +51,48 @@ __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, cons
   float acc[DEC_PER_CTA];
 #pragma unroll
   for (int oi = 0; oi < DEC_PER_CTA; ++oi) acc[oi] = 0.f;
-  // strain index of (output oi, tap k): top0 + oi*D - k; below n0 it lives in the f0 ring, below 0 it is zero
-  const long long rel0 = top0 - n0;                        // index relative to the pushed buffer (may be negative)
-  int ring_base = (int)(((n0 % rlen0) + rlen0) % rlen0);   // ring slot of stream sample n0
+  // The CTA's outputs read the contiguous strain span [top0 - 2c, top0 + (DEC_PER_CTA-1) D] (<= 4545 samples for D = 64):
+  // stage it in shared memory with one round of coalesced loads (below n0 it lives in the f0 ring, below 0 it is zero),
+  // then every (output, tap) product reads shared memory.  win[i] = d[top0 - 2c + i].
+  __shared__ float win[DEC_WIN];
+  const long long base = top0 - 2LL * r.c;                 // stream index of win[0]
+  const int nwin = ntap + (DEC_PER_CTA - 1) * D;
+  const int ring_base = (int)(((n0 % rlen0) + rlen0) % rlen0);   // ring slot of stream sample n0
+  auto strain_at = [&](long long idx) {
+    const long long rel = idx - n0;
+    if (rel >= 0) return sd[rel];
+    if (idx < 0) return 0.f;
+    long long sl = ring_base + rel;                        // rel in (-rlen0, 0): one wrap at most
+    if (sl < 0) sl += rlen0;
+    return ring0[sl];
+  };
+  if (nwin > DEC_WIN) {
+    // very long filters (n_down * D beyond the staged window): read the strain directly
+    for (int k = threadIdx.x; k < ntap; k += 256) {
+      const float t = taps[k];
+#pragma unroll
+      for (int oi = 0; oi < DEC_PER_CTA; ++oi) acc[oi] = fmaf(t, strain_at(top0 + (long long)oi * D - k), acc[oi]);
+    }
+  } else {
+  for (int i = threadIdx.x; i < nwin; i += 256) {
+    const long long idx = base + i, rel = idx - n0;
+    float v;
+    if (rel >= 0) v = sd[rel];
+    else if (idx < 0) v = 0.f;
+    else {
+      long long sl = ring_base + rel;                      // rel in (-rlen0, 0): one wrap at most
+      if (sl < 0) sl += rlen0;
+      v = ring0[sl];
+    }
+    win[i] = v;
+  }
+  __syncthreads();
   for (int k = threadIdx.x; k < ntap; k += 256) {
     const float t = taps[k];
+    const int w0 = 2 * r.c - k;                            // tap k of output oi reads d[top0 + oi D - k] = win[w0 + oi D]
 #pragma unroll
-    for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
-      const long long rel = rel0 + (long long)oi * D - k;
-      float v;
-      if (rel >= 0) v = sd[rel];
-      else if (rel + n0 < 0) v = 0.f;
-      else {
-        long long sl = ring_base + rel;                    // rel in (-rlen0, 0): one wrap at most
-        if (sl < 0) sl += rlen0;
-        v = ring0[sl];
-      }
-      acc[oi] = fmaf(t, v, acc[oi]);
-    }
+    for (int oi = 0; oi < DEC_PER_CTA; ++oi) acc[oi] = fmaf(t, win[w0 + oi * D], acc[oi]);
+  }
   }
 #pragma unroll
   for (int oi = 0; oi < DEC_PER_CTA; ++oi) {
