@@ -181,10 +181,23 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   const float *yr = rw->ysrc + (size_t)det * rw->ydet_stride;
   const int nseg = rw->nseg;
   const size_t yseg = (size_t)rw->yseg_stride;
-  auto load_y = [&](int sl) {                              // split-K partial sums added in segment order
-    float v = yr[(size_t)sl * ypitch];
-    for (int sg = 1; sg < nseg; ++sg) v += yr[sg * yseg + (size_t)sl * ypitch];
-    return v;
+  // 4 ring columns at a time: all (column, tap segment) loads are issued before any add; the split-K partial sums are
+  // then added in segment order (deterministic, same order for every caller)
+  auto load_y4 = [&](const int (&sl)[4], const bool (&ok)[4], float (&v)[4]) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) v[i] = 0.f;
+    for (int sg0 = 0; sg0 < nseg; sg0 += 4) {
+      float t[4][4];
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+          t[i][j] = (ok[i] && sg0 + j < nseg) ? yr[(size_t)(sg0 + j) * yseg + (size_t)sl[i] * ypitch] : 0.f;
+#pragma unroll
+      for (int j = 0; j < 4; ++j)
+#pragma unroll
+        for (int i = 0; i < 4; ++i) v[i] += t[i][j];
+    }
   };
   void *yup = rw->yup;
   const size_t plane_stride = (size_t)rw->yup_plane_stride;
@@ -197,11 +210,14 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   if (G == 0) {
     for (int c = warp; c < wg; c += 4 * nwarp) {
       float v[4];
+      int sl[4];
+      bool ok[4];
 #pragma unroll
       for (int i = 0; i < 4; ++i) {
-        v[i] = (active && c + i * nwarp < wg) ? load_y(slot) : 0.f;
+        sl[i] = slot; ok[i] = active && c + i * nwarp < wg;
         slot += nwarp; if (slot >= ylen) slot -= ylen;
       }
+      load_y4(sl, ok, v);
 #pragma unroll
       for (int i = 0; i < 4; ++i)
         if (active && c + i * nwarp < wg) up_store<HALF_PLANES>(yup, out0 + (size_t)(c + i * nwarp) * kpitch, plane_stride, v[i]);
@@ -210,11 +226,14 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
   }
   for (int c = warp; c < wg; c += 4 * nwarp) {            // 4 independent loads in flight per warp
     float v[4];
+    int sl[4];
+    bool ok[4];
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
-      v[i] = (active && c + i * nwarp < wg) ? load_y(slot) : 0.f;
+      sl[i] = slot; ok[i] = active && c + i * nwarp < wg;
       slot += nwarp; if (slot >= ylen) slot -= ylen;
     }
+    load_y4(sl, ok, v);
 #pragma unroll
     for (int i = 0; i < 4; ++i) if (c + i * nwarp < wg) buf[0][c + i * nwarp][lane] = v[i];
   }
@@ -225,7 +244,8 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
     // Output c (relative to lo_{h-1}) has input index qq = (r0 + c) >> lf relative to floor(lo_{h-1}/f) and phase
     // (r0 + c) & (f-1); in[qq] sits at buffer index qq + 8.  Each warp takes a run of consecutive qq, UP_RUN at a time,
     // with the run's inputs held in registers: ~3 shared loads per 16 FMA, no per-tap index arithmetic.
-    const int nq = ((r0 + wout - 1) >> lf) + 1, per = (nq + nwarp - 1) / nwarp;
+    // runs of UP_RUN inputs per warp (a multiple of UP_RUN each, so only the last warp's last run is ragged)
+    const int nq = ((r0 + wout - 1) >> lf) + 1, per = ((nq + nwarp - 1) / nwarp + UP_RUN - 1) / UP_RUN * UP_RUN;
     const int qa = warp * per, qb = min(qa + per, nq);
     const float(*in)[32] = buf[cur];
     float(*out)[32] = buf[cur ^ 1];
@@ -250,22 +270,40 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
           }
           odd[u] = v0 + v1;
         }
+        const bool full = nrun == UP_RUN && cbase >= 0 && cbase + 2 * UP_RUN <= wout;    // warp-uniform
         if (h == 1) {
           size_t o = out0 + (size_t)max(cbase, 0) * kpitch;
+          if (full) {
+            if (active) {
+#pragma unroll
+              for (int u = 0; u < UP_RUN; ++u) {
+                up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]);
+                up_store<HALF_PLANES>(yup, o + kpitch, plane_stride, odd[u]);
+                o += 2 * (size_t)kpitch;
+              }
+            }
+          } else {
+#pragma unroll
+            for (int u = 0; u < UP_RUN; ++u) {
+              const int c0 = cbase + 2 * u;
+              if (u < nrun && active) {
+                if (c0 >= 0 && c0 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]); o += kpitch; }
+                if (c0 + 1 >= 0 && c0 + 1 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, odd[u]); o += kpitch; }
+              }
+            }
+          }
+        } else if (full) {
 #pragma unroll
           for (int u = 0; u < UP_RUN; ++u) {
-            const int c0 = cbase + 2 * u;
-            if (u < nrun && active) {
-              if (c0 >= 0 && c0 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]); o += kpitch; }
-              if (c0 + 1 >= 0 && c0 + 1 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, odd[u]); o += kpitch; }
-            }
+            out[cbase + 2 * u][lane] = X[u + 7];                                 // phase 0: the copy of Eq. 8 case 1
+            out[cbase + 2 * u + 1][lane] = odd[u];
           }
         } else {
 #pragma unroll
           for (int u = 0; u < UP_RUN; ++u) {
             const int c0 = cbase + 2 * u;
             if (u < nrun) {
-              if (c0 >= 0 && c0 < wout) out[c0][lane] = X[u + 7];          // phase 0: the copy of Eq. 8 case 1
+              if (c0 >= 0 && c0 < wout) out[c0][lane] = X[u + 7];
               if (c0 + 1 >= 0 && c0 + 1 < wout) out[c0 + 1][lane] = odd[u];
             }
           }
