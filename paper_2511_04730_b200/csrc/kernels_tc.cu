@@ -212,14 +212,17 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 static constexpr int KS = 128;                                // taps per strip chunk (2 U stages)
 static constexpr int KSEG_MAX = 1024;                         // taps per unit (split-K segment)
 static constexpr int MAX_SUB = 2;
-static constexpr int STRIP_BYTES = (TILE_N + KS) * 16;        // one sub-tile, one plane, one buffer: 4096 B
-static constexpr int XWIN = TILE_N + KSEG_MAX + 8;            // staged strain window per sub-tile (floats)
+static constexpr int SUB_W = 256;                             // widest sub-tile: one MMA of N = 256 (operand reads < math cycles)
+static constexpr int STRIP_BYTES = (SUB_W + KS) * 16;         // one sub-tile, one plane, one buffer: 6144 B
+static constexpr int XWIN = SUB_W + KSEG_MAX + 8;             // staged strain window per sub-tile (floats)
 static constexpr int CORR_THREADS = 320;                      // warps: 0 TMA, 1 MMA, 2-5 epilogue, 6-9 strip builders
 
 struct TcCorrUnit {
   int cls, row0, k0, k1;                                      // taps [k0, k1), multiples of 64
   int seg, nsub;
   int det[MAX_SUB], col0[MAX_SUB];
+  int nt[MAX_SUB];                                            // MMA N of the sub-tile: columns rounded up to 16; one sub-tile
+                                                              // of up to 256 columns, or two of up to 128 (256 TMEM columns per unit)
 };
 
 int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
@@ -275,9 +278,9 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       int stage = 0; uint32_t phase = 0; int it = 0, chunk_it = 0;
       for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
         const TcCorrUnit *u = &units[ui];
-        const int nsub = u->nsub, ncols = classes[u->cls].ncols, k0 = u->k0, k1 = u->k1;
-        const uint32_t idesc0 = idesc_f16_f32(TILE_M, min(TILE_N, (ncols - u->col0[0] + 15) & ~15));
-        const uint32_t idesc1 = idesc_f16_f32(TILE_M, nsub > 1 ? min(TILE_N, (ncols - u->col0[1] + 15) & ~15) : 16);
+        const int nsub = u->nsub, k0 = u->k0, k1 = u->k1;
+        const uint32_t idesc0 = idesc_f16_f32(TILE_M, u->nt[0]);
+        const uint32_t idesc1 = idesc_f16_f32(TILE_M, nsub > 1 ? u->nt[1] : 16);
         const int buf = it & 1;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
@@ -330,7 +333,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
         const int p0 = (int)(((first % c.rlen) + c.rlen) % c.rlen);
         const float *x = c.ring2 + (size_t)u->det[sb] * c.ring_det_stride + p0 + k0;
         float *w = xwin + sb * XWIN;
-        const int nw = TILE_N + klen + 8;
+        const int nw = u->nt[sb] + klen + 8;
         for (int i = tid; i < nw; i += 4 * 128) {
           float v[4];
 #pragma unroll
@@ -343,8 +346,8 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       for (int kc = 0; kc < klen; kc += KS, ++chunk_it) {
         const int sbuf = chunk_it & 1;
         mbar_wait(&sempty[sbuf], ((chunk_it >> 1) & 1) ^ 1);
-        const int n_ent = TILE_N + min(KS, klen - kc);            // entry e = 8 m + r holds x[kc + e .. kc + e + 8)
         for (int sb = 0; sb < nsub; ++sb) {
+          const int n_ent = u->nt[sb] + min(KS, klen - kc);        // entry e = 8 m + r holds x[kc + e .. kc + e + 8)
           uint8_t *dst = strips + (sbuf * MAX_SUB + sb) * PLANES * STRIP_BYTES;
           const float *xs = xwin + sb * XWIN + kc;
           for (int e = tid; e < n_ent; e += 128) {
@@ -388,7 +391,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       for (int sb = 0; sb < nsub; ++sb) {
         const int col0 = u->col0[sb];
         float *yr = c.yring + (size_t)u->seg * c.yseg_stride + (size_t)u->det[sb] * c.ydet_stride + row;
-        const int NT = min(TILE_N, (ncols - col0 + 15) & ~15);
+        const int NT = u->nt[sb];
         const int slot0 = (int)((n0 / c.D + c.H + col0 + 64) % ylen);
         for (int cc = 0; cc < NT; cc += 32) {
           uint32_t v[32];
@@ -531,19 +534,28 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     const int nseg = tc_k_segments(c.Npad);
     const int kseg = ((c.Npad + nseg - 1) / nseg + BK - 1) / BK * BK;
-    std::vector<std::pair<int, int>> subs;
+    struct Sub { int det, c0, w; };
+    std::vector<Sub> subs;
     for (int det = 0; det < n_det; ++det)
-      for (int c0 = 0; c0 < c.ncols; c0 += TILE_N) subs.push_back({det, c0});
+      for (int c0 = 0; c0 < c.ncols;) {                      // wide sub-tiles (<= 256 columns) while more than 128 remain
+        const int w = (c.ncols - c0 > TILE_N) ? std::min(SUB_W, c.ncols - c0) : c.ncols - c0;
+        subs.push_back({det, c0, w});
+        c0 += w;
+      }
     for (int r0 = 0; r0 < c.Lstack; r0 += TILE_M)
       for (int sg = 0; sg < nseg; ++sg) {
         const int k0 = sg * kseg, k1 = std::min(c.Npad, k0 + kseg);
         if (k0 >= k1) continue;
-        for (size_t s0 = 0; s0 < subs.size(); s0 += MAX_SUB) {
+        for (size_t s0 = 0; s0 < subs.size();) {
           TcCorrUnit u; memset(&u, 0, sizeof(u));
           u.cls = (int)ci; u.row0 = r0; u.k0 = k0; u.k1 = k1; u.seg = sg;
-          u.nsub = (int)std::min<size_t>(MAX_SUB, subs.size() - s0);
-          for (int i = 0; i < u.nsub; ++i) { u.det[i] = subs[s0 + i].first; u.col0[i] = subs[s0 + i].second; }
+          // one wide sub-tile, or two narrow ones, per unit (256 accumulator columns)
+          u.nsub = (subs[s0].w > TILE_N || s0 + 1 >= subs.size() || subs[s0 + 1].w > TILE_N) ? 1 : 2;
+          for (int i = 0; i < u.nsub; ++i) {
+            u.det[i] = subs[s0 + i].det; u.col0[i] = subs[s0 + i].c0; u.nt[i] = (subs[s0 + i].w + 15) & ~15;
+          }
           cu.push_back(u);
+          s0 += u.nsub;
         }
       }
   }
@@ -575,7 +587,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
   std::vector<int> cbegin, rbegin;
-  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)u.nsub * (u.k1 - u.k0) + 128; }, cbegin);
+  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
   lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * ((rb[t.bank].Kpad + BK - 1) / BK + 1); }, rbegin);
   if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
