@@ -215,7 +215,7 @@ static constexpr int MAX_SUB = 2;
 static constexpr int SUB_W = 256;                             // widest sub-tile: one MMA of N = 256 (operand reads < math cycles)
 static constexpr int STRIP_BYTES = (SUB_W + KS) * 16;         // one sub-tile, one plane, one buffer: 6144 B
 static constexpr int XWIN = SUB_W + KSEG_MAX + 8;             // staged strain window per sub-tile (floats)
-static constexpr int CORR_THREADS = 320;                      // warps: 0 TMA, 1 MMA, 2-5 epilogue, 6-9 strip builders
+static constexpr int CORR_THREADS = 448;                      // warps: 0 TMA, 1 MMA, 2-5 + 10-13 epilogue, 6-9 strip builders
 
 struct TcCorrUnit {
   int cls, row0, k0, k1;                                      // taps [k0, k1), multiples of 64
@@ -245,7 +245,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&ufull[i], 1); mbar_init(&uempty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&sfull[i], 4); mbar_init(&sempty[i], 1); mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 4); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&sfull[i], 4); mbar_init(&sempty[i], 1); mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 8); }
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -317,7 +317,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
         mma_commit(&tfull[buf]);
       }
     }
-  } else if (warp >= 6) {
+  } else if (warp >= 6 && warp < 10) {
     // ===== strip builders (128 threads): stage the strain windows of a unit, then build its strips chunk by chunk
     const int tid = threadIdx.x - 192;
     const long long n0 = *n0_ptr;
@@ -373,35 +373,55 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       }
     }
   } else {
-    // ===== epilogue (warps 2-5): thread = basis row (TMEM lane); partial sums of this tap segment -> plane `seg` of the Y ring
+    // ===== epilogue (warps 2-5 and 10-13): thread = basis row (TMEM lane); the two warp groups take alternate chunks of
+    // 32 columns; partial sums of this tap segment -> plane `seg` of the Y ring (time-major: 128 B per warp store)
     const int q = warp & 3;
+    const int grp = warp >= 10 ? 1 : 0;
     const long long n0 = *n0_ptr;
     int it = 0;
     for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
       const TcCorrUnit *u = &units[ui];
       const CorrClass &c = classes[u->cls];
       const int nsub = u->nsub, buf = it & 1;
-      const int ylen = c.ylen, Lpad = c.Lpad, ncols = c.ncols;
+      const int ylen = c.ylen, ncols = c.ncols;
+      const size_t Lpad = (size_t)c.Lpad;
       const float sc = c.u_scale_inv;
       const int row = u->row0 + q * 32 + lane;
       const bool row_ok = row < c.Lstack;
+      const long long jbase = n0 / c.D + c.H + 64;
+      float *ybase = c.yring + (size_t)u->seg * c.yseg_stride + row;
       mbar_wait(&tfull[buf], (it >> 1) & 1);
       tc_fence_after_sync();
       const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + buf * (MAX_SUB * TILE_N);
       for (int sb = 0; sb < nsub; ++sb) {
-        const int col0 = u->col0[sb];
-        float *yr = c.yring + (size_t)u->seg * c.yseg_stride + (size_t)u->det[sb] * c.ydet_stride + row;
-        const int NT = u->nt[sb];
-        const int slot0 = (int)((n0 / c.D + c.H + col0 + 64) % ylen);
-        for (int cc = 0; cc < NT; cc += 32) {
+        const int col0 = u->col0[sb], NT = u->nt[sb];
+        float *yr = ybase + (size_t)u->det[sb] * c.ydet_stride;
+        const int slot0 = (int)((jbase + col0) % ylen);
+        const int nvalid = min(NT, ncols - col0);                 // columns of this sub-tile that exist
+        for (int cc = grp * 32; cc < nvalid; cc += 64) {
           uint32_t v[32];
           tmem_ld_32x32(taddr + sb * TILE_N + cc, v);
           tmem_ld_wait();
+          int slot = slot0 + cc;
+          if (slot >= ylen) slot -= ylen;
+          float *p = yr + (size_t)slot * Lpad;
+          float *const pend = yr + (size_t)ylen * Lpad;
+          if (row_ok) {
+            if (cc + 32 <= nvalid) {
 #pragma unroll
-          for (int i = 0; i < 32; ++i) {
-            int slot = slot0 + cc + i;
-            if (slot >= ylen) slot -= ylen;
-            if (col0 + cc + i < ncols && row_ok) yr[(size_t)slot * Lpad] = __uint_as_float(v[i]) * sc;
+              for (int i = 0; i < 32; ++i) {
+                *p = __uint_as_float(v[i]) * sc;
+                p += Lpad;
+                if (p >= pend) p -= (size_t)ylen * Lpad;
+              }
+            } else {
+#pragma unroll
+              for (int i = 0; i < 32; ++i) {
+                if (cc + i < nvalid) *p = __uint_as_float(v[i]) * sc;
+                p += Lpad;
+                if (p >= pend) p -= (size_t)ylen * Lpad;
+              }
+            }
           }
         }
       }
