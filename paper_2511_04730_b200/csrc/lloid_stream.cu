@@ -148,31 +148,52 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   }
   dp.total_out = out_begin;
 
-  // ---- geometry classes: slices with equal (D, N, delay, H) share one Hankel operand; stack their U rows
-  typedef std::tuple<int, int, long long, int> Key;
-  std::map<Key, int> class_of;
-  std::vector<std::vector<std::pair<int, int>>> members;     // class -> (bank, slice)
-  std::vector<std::vector<int>> row_off(n_banks);
+  // ---- geometry classes (slices of equal rate stacked across banks).  Slices at one rate with the same
+  //      upsample halo H whose tap windows [delay, delay + N) nearly coincide share ONE Hankel operand: the class window
+  //      is the union [dmin, emax), every member's U is placed at column emax - (delay_i + N_i) and zero padded, as long
+  //      as the union stays within 1.25x of the shortest member (so no member's contraction grows by more than 25 %).
+  struct Member { int b, i, L; long long d, e; };
+  std::map<std::pair<int, int>, std::vector<Member>> by_rate;   // (D, H) -> slices
   for (int b = 0; b < n_banks; ++b) {
     const lloid_bank *bk = s->banks[b];
-    row_off[b].resize(bk->S);
     for (int i = 0; i < bk->S; ++i) {
       const SliceInfo &si = bk->slices[i];
-      Key key(si.D, si.N, si.delay, bk->groups[si.group].H);
-      auto it = class_of.find(key);
-      int c;
-      if (it == class_of.end()) {
-        c = (int)s->classes.size(); class_of[key] = c; members.emplace_back();
-        CorrClass cc; memset(&cc, 0, sizeof(cc));
-        const RateDev &r = dp.r[rate_index[si.D]];
-        cc.ring2 = r.ring2; cc.ring_det_stride = 2LL * r.rlen; cc.rlen = r.rlen; cc.lag = r.lag; cc.D = si.D;
-        cc.N = si.N; cc.Npad = (si.N + 63) / 64 * 64; cc.H = bk->groups[si.group].H; cc.delay = si.delay;
-        cc.ncols = B / si.D; cc.ylen = B / si.D + 32; cc.u_scale_inv = 1.f;
-        s->classes.push_back(cc);
-      } else c = it->second;
-      row_off[b][i] = s->classes[c].Lstack;
-      s->classes[c].Lstack += si.L;
-      members[c].push_back({b, i});
+      by_rate[{si.D, bk->groups[si.group].H}].push_back({b, i, si.L, si.delay, si.delay + si.N});
+    }
+  }
+  std::vector<std::vector<Member>> members;                      // class -> members
+  std::vector<std::vector<int>> row_off(n_banks), cls_of(n_banks);
+  for (int b = 0; b < n_banks; ++b) { row_off[b].resize(s->banks[b]->S); cls_of[b].resize(s->banks[b]->S); }
+  for (auto &kv : by_rate) {
+    std::vector<Member> &v = kv.second;
+    std::stable_sort(v.begin(), v.end(), [](const Member &x, const Member &y) { return x.d != y.d ? x.d < y.d : x.e < y.e; });
+    size_t i0 = 0;
+    while (i0 < v.size()) {
+      long long dmin = v[i0].d, emax = v[i0].e, nmin = v[i0].e - v[i0].d;
+      size_t i1 = i0 + 1;
+      for (; i1 < v.size(); ++i1) {
+        const long long d2 = std::min(dmin, v[i1].d), e2 = std::max(emax, v[i1].e), n2 = std::min(nmin, v[i1].e - v[i1].d);
+        if ((e2 - d2) * 4 > n2 * 5) break;
+        dmin = d2; emax = e2; nmin = n2;
+      }
+      const int c = (int)s->classes.size();
+      CorrClass cc; memset(&cc, 0, sizeof(cc));
+      const int D = kv.first.first;
+      const RateDev &r = dp.r[rate_index[D]];
+      cc.ring2 = r.ring2; cc.ring_det_stride = 2LL * r.rlen; cc.rlen = r.rlen; cc.lag = r.lag; cc.D = D;
+      cc.N = (int)(emax - dmin); cc.Npad = (cc.N + 63) / 64 * 64; cc.H = kv.first.second; cc.delay = dmin;
+      cc.ncols = B / D; cc.ylen = B / D + 32; cc.u_scale_inv = 1.f;
+      members.emplace_back();
+      // keep bank order inside the class (deterministic row layout)
+      std::vector<Member> mm(v.begin() + i0, v.begin() + i1);
+      std::stable_sort(mm.begin(), mm.end(), [](const Member &x, const Member &y) { return x.b != y.b ? x.b < y.b : x.i < y.i; });
+      for (const Member &m : mm) {
+        row_off[m.b][m.i] = cc.Lstack; cls_of[m.b][m.i] = c;
+        cc.Lstack += m.L;
+        members.back().push_back(m);
+      }
+      s->classes.push_back(cc);
+      i0 = i1;
     }
   }
   std::vector<CorrTile> tiles;
@@ -181,9 +202,12 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     cc.Lpad = (cc.Lstack + 127) / 128 * 128;
     std::vector<float> U((size_t)cc.Lpad * cc.Npad, 0.f);
     int row = 0;
-    for (auto &m : members[c]) {
-      const SliceInfo &si = s->banks[m.first]->slices[m.second];
-      for (int l = 0; l < si.L; ++l, ++row) memcpy(&U[(size_t)row * cc.Npad], &si.U[(size_t)l * si.N], sizeof(float) * si.N);
+    double alg = 0;
+    for (const Member &m : members[c]) {
+      const SliceInfo &si = s->banks[m.b]->slices[m.i];
+      const long long off = (cc.delay + cc.N) - m.e;            // class column of the member's oldest tap
+      for (int l = 0; l < si.L; ++l, ++row) memcpy(&U[(size_t)row * cc.Npad + off], &si.U[(size_t)l * si.N], sizeof(float) * si.N);
+      alg += (double)si.L * si.N;
     }
     if (s->precision == LLOID_PREC_FP32_FFMA) {
       float *p; CK(dev_upload(s, &p, U)); cc.U32 = p;
@@ -207,7 +231,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     for (int r0 = 0; r0 < cc.Lstack; r0 += 64)
       for (int c0 = 0; c0 < cc.ncols; c0 += 64) tiles.push_back({(int)c, r0, c0});
     s->work[0] += 2.0 * cc.Lpad * cc.Npad * cc.ncols * n_det;               // executed (padded) flop, one pass
-    s->work[2] += 2.0 * cc.Lstack * (double)cc.N * cc.ncols * n_det;
+    s->work[2] += 2.0 * alg * cc.ncols * n_det;
     s->work[5] += (double)cc.Lpad * cc.Npad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
     s->work[6] += 2.0 * 4.0 * cc.Lstack * cc.ncols * n_det;
   }
@@ -253,7 +277,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     for (int g = 0; g < bk->G; ++g) { if (g > 0) up_out += bk->groups[g - 1].rate; }
     for (int i = 0; i < bk->S; ++i) {
       const SliceInfo &si = bk->slices[i];
-      const CorrClass &cc = s->classes[class_of[Key(si.D, si.N, si.delay, bk->groups[si.group].H)]];
+      const CorrClass &cc = s->classes[cls_of[b][i]];
       std::vector<int> key;
       key.push_back(si.D);
       for (int h = 1; h <= si.group; ++h) key.push_back((int)std::lround(std::log2((double)bk->groups[h].f)));

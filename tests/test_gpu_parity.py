@@ -187,3 +187,23 @@ def test_two_streams_share_banks_and_errors():
         lib.lloid_stream_create([h], 1, 101)            # not a multiple of the largest decimation factor (2)
     assert e.value.code == lib.LLOID_EINVAL
     lib.lloid_stream_destroy(s1); lib.lloid_stream_destroy(s2); lib.lloid_bank_destroy(h)
+
+
+@pytest.mark.parametrize("precision", [2, 0])
+def test_merged_geometry_classes(precision):
+    """Two banks whose slices at 1024 Hz and 512 Hz have slightly different tap counts and delays: their windows are
+    merged into one Hankel operand with per-member column offsets (DESIGN.md section 5 "stacking")."""
+    _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import lloid_snr
+    from workloads import make_strain, random_bank
+    banks = [random_bank(31, 20, [(2048, 512, 10), (1024, 768, 12), (512, 640, 9)]).as_f32(),
+             random_bank(32, 28, [(2048, 512, 7), (1024, 800, 11), (512, 600, 8)]).as_f32()]
+    B, n_push = 512, 8
+    strain = np.stack([make_strain(310, B * n_push)])
+    for bi, bank in enumerate(banks):
+        rho_gpu, _ = run_gpu(banks, strain, B, precision, want_bank=bi)
+        ref = lloid_snr(bank, strain[0])
+        emax, erms = check_snr(rho_gpu[0], ref, TOL[precision])
+        print(f"merged classes bank {bi} precision {precision}: max err {emax:.3e}")
+        assert emax <= TOL[precision]
