@@ -133,7 +133,8 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 // ------------------------------------------------------------------------------------------------
 #define UP_RUN 8
 struct UpTaps2 { float t[16]; };   // g_2[2k+1], k = 0..15: the 16 non-zero taps of the x2 interpolation phase (Eq. 7)
-#define UP_MAXW 168   // widest staged level: chunk/2 + 2*8 + ... <= 256/2 + 33
+#define UP_CHUNK 512  // f0 samples per CTA
+#define UP_MAXW (UP_CHUNK / 2 + 40)   // widest staged level: chunk/2 + 2*8 + 1 (+ slack)
 template <int HALF_PLANES>
 __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_stride, float v) {
   if (HALF_PLANES == 0) {
@@ -146,11 +147,12 @@ __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_strid
 }
 
 template <int HALF_PLANES>
-__global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
+__global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
                                                           const float *__restrict__ uptaps,
                                                           const int *__restrict__ uptap_off,
                                                           const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
-  __shared__ float buf[2][UP_MAXW][32];
+  extern __shared__ __align__(16) float up_dyn[];
+  float(*buf)[UP_MAXW][32] = reinterpret_cast<float(*)[UP_MAXW][32]>(up_dyn);
   __shared__ int s_r0[LLOID_MAX_GROUPS + 1], s_w[LLOID_MAX_GROUPS + 1], s_lf[LLOID_MAX_GROUPS + 1], s_slot0;
   const UpItem *it = &items[blockIdx.y];
   const int det = blockIdx.z;
@@ -341,6 +343,14 @@ __global__ void __launch_bounds__(256, 4) upsample_kernel(const UpItem *__restri
 cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
                             const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
+  const int smem = 2 * UP_MAXW * 32 * (int)sizeof(float);
+  static bool attr = false;
+  if (!attr) {
+    cudaFuncSetAttribute(upsample_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(upsample_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    cudaFuncSetAttribute(upsample_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+    attr = true;
+  }
   static UpTaps2 t2;                                     // Eq. 4 with f = 2, c = 16 (same float64 -> fp32 values as uptaps)
   static bool have = false;
   if (!have) {
@@ -350,9 +360,9 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
     }
     have = true;
   }
-  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else upsample_kernel<2><<<grid, 256, 0, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else upsample_kernel<2><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   return cudaGetLastError();
 }
 

@@ -109,7 +109,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
-  s->up_chunk = std::min(B, 256);
+  s->up_chunk = std::min(B, 512);                   // = UP_CHUNK of kernels_stream.cu
   memset(s->work, 0, sizeof(s->work));
   int dev = 0; cudaDeviceProp prop;
   CK(cudaGetDevice(&dev));
