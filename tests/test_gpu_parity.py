@@ -207,3 +207,22 @@ def test_merged_geometry_classes(precision):
         emax, erms = check_snr(rho_gpu[0], ref, TOL[precision])
         print(f"merged classes bank {bi} precision {precision}: max err {emax:.3e}")
         assert emax <= TOL[precision]
+
+
+@pytest.mark.parametrize("precision", [2, 0])
+def test_large_decimation_and_single_big_upsample_stage(precision):
+    """A bank that jumps from 2048 Hz straight to 16 Hz (D = 128): 8193-tap decimator (the kernel's direct-read path, its
+    staged window only covers D <= 64) and ONE x128 upsample stage (the generic-factor path of the polyphase kernel)."""
+    _torch_cuda()
+    from oracle import lloid_snr
+    from workloads import make_strain, random_bank
+    bank = random_bank(41, 24, [(2048, 8192, 14), (16, 96, 10)]).as_f32()
+    B, n_push = 1024, 12
+    strain = np.stack([make_strain(410 + d, B * n_push) for d in range(2)])
+    rho_gpu, peaks = run_gpu([bank], strain, B, precision)
+    for det in range(2):
+        ref = lloid_snr(bank, strain[det])
+        emax, erms = check_snr(rho_gpu[det], ref, TOL[precision])
+        print(f"D=128 bank det {det} precision {precision}: max err {emax:.3e}")
+        assert emax <= TOL[precision]
+        check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0))
