@@ -11,6 +11,7 @@
 #include <algorithm>
 #include <cstring>
 #include <queue>
+#include <type_traits>
 
 #include "lloid_internal.h"
 #include "tc_ptx.cuh"
@@ -106,20 +107,20 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         for (int kb = 0; kb < nkb; ++kb) {
           mbar_wait(&full[stage], phase);
           tc_fence_after_sync();
-          const uint32_t s = smem_u32(smem + stage * STAGE_BYTES);
+          // one base descriptor per stage; every operand tile / K step is a constant added to its 16-byte address field
+          const uint64_t db = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
           const int nk = min(BK / 16, (Kpad - kb * BK) / 16);       // K is padded to 16, the last 64-wide box is zero-filled
 #pragma unroll
           for (int k = 0; k < BK / 16; ++k) {
             if (k >= nk) break;
-            const uint32_t ko = k * 32;
             const bool acc = (kb | k) != 0;
-            const uint64_t re_hi = desc_kmajor_sw128(s + 0 * TILE_BYTES + ko), im_hi = desc_kmajor_sw128(s + 1 * TILE_BYTES + ko),
-                           y_hi = desc_kmajor_sw128(s + 2 * TILE_BYTES + ko);
+            const uint64_t re_hi = db + ((0 * TILE_BYTES + k * 32) >> 4), im_hi = db + ((1 * TILE_BYTES + k * 32) >> 4),
+                           y_hi = db + ((2 * TILE_BYTES + k * 32) >> 4);
             mma_f16_ss(d_re, re_hi, y_hi, idesc, acc);
             mma_f16_ss(d_im, im_hi, y_hi, idesc, acc);
             if (PLANES == 2) {
-              const uint64_t re_lo = desc_kmajor_sw128(s + 3 * TILE_BYTES + ko), im_lo = desc_kmajor_sw128(s + 4 * TILE_BYTES + ko),
-                             y_lo = desc_kmajor_sw128(s + 5 * TILE_BYTES + ko);
+              const uint64_t re_lo = db + ((3 * TILE_BYTES + k * 32) >> 4), im_lo = db + ((4 * TILE_BYTES + k * 32) >> 4),
+                             y_lo = db + ((5 * TILE_BYTES + k * 32) >> 4);
               mma_f16_ss(d_re, re_hi, y_lo, idesc, true);
               mma_f16_ss(d_im, im_hi, y_lo, idesc, true);
               mma_f16_ss(d_re, re_lo, y_hi, idesc, true);
@@ -211,18 +212,21 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 // ------------------------------------------------------------------------------------------------
 static constexpr int KS = 128;                                // taps per strip chunk (2 U stages)
 static constexpr int KSEG_MAX = 1024;                         // taps per unit (split-K segment)
-static constexpr int MAX_SUB = 2;
+static constexpr int MAX_SUB = 4;                             // sub-tiles per unit, packed into 256 accumulator columns
+static constexpr int UNIT_N = 256;                            // accumulator columns per unit (x2 TMEM buffers)
 static constexpr int SUB_W = 256;                             // widest sub-tile: one MMA of N = 256 (operand reads < math cycles)
-static constexpr int STRIP_BYTES = (SUB_W + KS) * 16;         // one sub-tile, one plane, one buffer: 6144 B
-static constexpr int XWIN = SUB_W + KSEG_MAX + 8;             // staged strain window per sub-tile (floats)
+static constexpr int STRIP_PLANE = (UNIT_N + MAX_SUB * KS) * 16;   // strips of all sub-tiles of a unit, one plane, one buffer: 12 KB
+static constexpr int XWIN_TOTAL = UNIT_N + MAX_SUB * (KSEG_MAX + 8);  // staged strain windows of all sub-tiles (floats)
 static constexpr int CORR_THREADS = 448;                      // warps: 0 TMA, 1 MMA, 2-5 + 10-13 epilogue, 6-9 strip builders
 
 struct TcCorrUnit {
   int cls, row0, k0, k1;                                      // taps [k0, k1), multiples of 64
   int seg, nsub;
   int det[MAX_SUB], col0[MAX_SUB];
-  int nt[MAX_SUB];                                            // MMA N of the sub-tile: columns rounded up to 16; one sub-tile
-                                                              // of up to 256 columns, or two of up to 128 (256 TMEM columns per unit)
+  int nt[MAX_SUB];                                            // MMA N of the sub-tile: columns rounded up to 16, sum <= UNIT_N
+  int tcol[MAX_SUB];                                          // first accumulator column of the sub-tile (prefix sum of nt)
+  int soff[MAX_SUB];                                          // byte offset of the sub-tile's strip inside a plane: 16 * (tcol + sb * KS)
+  int xoff[MAX_SUB];                                          // float offset of the sub-tile's staged strain window
 };
 
 int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
@@ -235,9 +239,9 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t *strips = smem + STAGES * STAGE_BYTES;                 // [2 buffers][MAX_SUB][PLANES][STRIP_BYTES]
-  float *xwin = (float *)(strips + 2 * MAX_SUB * PLANES * STRIP_BYTES);   // [MAX_SUB][XWIN]
-  uint64_t *bars = (uint64_t *)(xwin + MAX_SUB * XWIN);
+  uint8_t *strips = smem + STAGES * STAGE_BYTES;                 // [2 buffers][PLANES][STRIP_PLANE]
+  float *xwin = (float *)(strips + 2 * PLANES * STRIP_PLANE);    // [XWIN_TOTAL]
+  uint64_t *bars = (uint64_t *)(xwin + XWIN_TOTAL);
   uint64_t *ufull = bars, *uempty = bars + STAGES, *sfull = bars + 2 * STAGES, *sempty = sfull + 2, *tfull = sempty + 2,
            *tempty = tfull + 2;
   uint32_t *tmem_slot = (uint32_t *)(tempty + 2);
@@ -279,41 +283,52 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
         const TcCorrUnit *u = &units[ui];
         const int nsub = u->nsub, k0 = u->k0, k1 = u->k1;
-        const uint32_t idesc0 = idesc_f16_f32(TILE_M, u->nt[0]);
-        const uint32_t idesc1 = idesc_f16_f32(TILE_M, nsub > 1 ? u->nt[1] : 16);
+        uint32_t idesc[MAX_SUB], dcol[MAX_SUB], sdesc[MAX_SUB];
+#pragma unroll
+        for (int sb = 0; sb < MAX_SUB; ++sb) {
+          idesc[sb] = idesc_f16_f32(TILE_M, sb < nsub ? u->nt[sb] : 16);
+          dcol[sb] = sb < nsub ? u->tcol[sb] : 0;
+          sdesc[sb] = sb < nsub ? (uint32_t)(u->soff[sb] >> 4) : 0;
+        }
         const int buf = it & 1;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
-        const uint32_t d0 = tmem + buf * (MAX_SUB * TILE_N), d1 = d0 + TILE_N;
-        for (int kc = k0; kc < k1; kc += KS, ++chunk_it) {
-          const int sbuf = chunk_it & 1;
-          mbar_wait(&sfull[sbuf], (chunk_it >> 1) & 1);
-          tc_fence_after_sync();
-          const uint64_t xd = desc_kmajor_nosw(smem_u32(strips + sbuf * MAX_SUB * PLANES * STRIP_BYTES), 128, 128);
-          const int kend = min(kc + KS, k1);
-          for (int kb = kc; kb < kend; kb += BK) {
-            mbar_wait(&ufull[stage], phase);
+        const uint32_t d0 = tmem + buf * UNIT_N;
+        // the chunk / k loops, specialised on the number of sub-tiles so the single issuing thread runs straight-line code
+        auto issue = [&](auto ns_tag) {
+          constexpr int NS = decltype(ns_tag)::value;
+          for (int kc = k0; kc < k1; kc += KS, ++chunk_it) {
+            const int sbuf = chunk_it & 1;
+            mbar_wait(&sfull[sbuf], (chunk_it >> 1) & 1);
             tc_fence_after_sync();
-            const uint64_t ud = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
-            const uint64_t xk = xd + (uint64_t)(kb - kc);              // 16 B per tap
+            const uint64_t xd = desc_kmajor_nosw(smem_u32(strips + sbuf * PLANES * STRIP_PLANE), 128, 128);
+            const int kend = min(kc + KS, k1);
+            for (int kb = kc; kb < kend; kb += BK) {
+              mbar_wait(&ufull[stage], phase);
+              tc_fence_after_sync();
+              const uint64_t ud = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
+              const uint64_t xk = xd + (uint64_t)(kb - kc);              // 16 B per tap
 #pragma unroll
-            for (int k = 0; k < BK / 16; ++k) {
-              const bool acc = (kb > k0) || (k > 0);
-              const uint64_t u_hi = ud + 2 * k, u_lo = u_hi + (TILE_BYTES >> 4);
-              const uint64_t x0_hi = xk + 16 * k, x0_lo = x0_hi + (STRIP_BYTES >> 4);
-              mma_f16_ss(d0, u_hi, x0_hi, idesc0, acc);
-              if (PLANES == 2) { mma_f16_ss(d0, u_hi, x0_lo, idesc0, true); mma_f16_ss(d0, u_lo, x0_hi, idesc0, true); }
-              if (nsub > 1) {
-                const uint64_t x1_hi = x0_hi + (PLANES * STRIP_BYTES >> 4), x1_lo = x1_hi + (STRIP_BYTES >> 4);
-                mma_f16_ss(d1, u_hi, x1_hi, idesc1, acc);
-                if (PLANES == 2) { mma_f16_ss(d1, u_hi, x1_lo, idesc1, true); mma_f16_ss(d1, u_lo, x1_hi, idesc1, true); }
+              for (int k = 0; k < BK / 16; ++k) {
+                const bool acc = (kb > k0) || (k > 0);
+                const uint64_t u_hi = ud + 2 * k, u_lo = u_hi + (TILE_BYTES >> 4);
+#pragma unroll
+                for (int sb = 0; sb < NS; ++sb) {
+                  const uint64_t x_hi = xk + 16 * k + sdesc[sb], x_lo = x_hi + (STRIP_PLANE >> 4);
+                  mma_f16_ss(d0 + dcol[sb], u_hi, x_hi, idesc[sb], acc);
+                  if (PLANES == 2) { mma_f16_ss(d0 + dcol[sb], u_hi, x_lo, idesc[sb], true); mma_f16_ss(d0 + dcol[sb], u_lo, x_hi, idesc[sb], true); }
+                }
               }
+              mma_commit(&uempty[stage]);
+              if (++stage == STAGES) { stage = 0; phase ^= 1; }
             }
-            mma_commit(&uempty[stage]);
-            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+            mma_commit(&sempty[sbuf]);
           }
-          mma_commit(&sempty[sbuf]);
-        }
+        };
+        if (nsub == 1) issue(std::integral_constant<int, 1>());
+        else if (nsub == 2) issue(std::integral_constant<int, 2>());
+        else if (nsub == 3) issue(std::integral_constant<int, 3>());
+        else issue(std::integral_constant<int, 4>());
         mma_commit(&tfull[buf]);
       }
     }
@@ -332,7 +347,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
         const long long first = n0 / c.D + c.H + u->col0[sb] - c.delay - c.N + 1 + c.lag;
         const int p0 = (int)(((first % c.rlen) + c.rlen) % c.rlen);
         const float *x = c.ring2 + (size_t)u->det[sb] * c.ring_det_stride + p0 + k0;
-        float *w = xwin + sb * XWIN;
+        float *w = xwin + u->xoff[sb];
         const int nw = u->nt[sb] + klen + 8;
         for (int i = tid; i < nw; i += 4 * 128) {
           float v[4];
@@ -343,13 +358,20 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
         }
       }
       asm volatile("bar.sync 1, 128;" ::: "memory");
+      int nt_r[MAX_SUB], soff_r[MAX_SUB], xoff_r[MAX_SUB];        // the unit's sub-tile table in registers
+#pragma unroll
+      for (int sb = 0; sb < MAX_SUB; ++sb) {
+        nt_r[sb] = sb < nsub ? u->nt[sb] : 0; soff_r[sb] = sb < nsub ? u->soff[sb] : 0; xoff_r[sb] = sb < nsub ? u->xoff[sb] : 0;
+      }
       for (int kc = 0; kc < klen; kc += KS, ++chunk_it) {
         const int sbuf = chunk_it & 1;
         mbar_wait(&sempty[sbuf], ((chunk_it >> 1) & 1) ^ 1);
-        for (int sb = 0; sb < nsub; ++sb) {
-          const int n_ent = u->nt[sb] + min(KS, klen - kc);        // entry e = 8 m + r holds x[kc + e .. kc + e + 8)
-          uint8_t *dst = strips + (sbuf * MAX_SUB + sb) * PLANES * STRIP_BYTES;
-          const float *xs = xwin + sb * XWIN + kc;
+#pragma unroll
+        for (int sb = 0; sb < MAX_SUB; ++sb) {
+          if (sb >= nsub) break;
+          const int n_ent = nt_r[sb] + min(KS, klen - kc);         // entry e = 8 m + r holds x[kc + e .. kc + e + 8)
+          uint8_t *dst = strips + sbuf * PLANES * STRIP_PLANE + soff_r[sb];
+          const float *xs = xwin + xoff_r[sb] + kc;
           for (int e = tid; e < n_ent; e += 128) {
             float v[8];
 #pragma unroll
@@ -364,7 +386,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
               }
             }
             *reinterpret_cast<uint4 *>(dst + (size_t)e * 16) = *reinterpret_cast<uint4 *>(h);
-            if (PLANES == 2) *reinterpret_cast<uint4 *>(dst + STRIP_BYTES + (size_t)e * 16) = *reinterpret_cast<uint4 *>(l);
+            if (PLANES == 2) *reinterpret_cast<uint4 *>(dst + STRIP_PLANE + (size_t)e * 16) = *reinterpret_cast<uint4 *>(l);
           }
         }
         fence_proxy_async_smem();
@@ -392,7 +414,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
       float *ybase = c.yring + (size_t)u->seg * c.yseg_stride + row;
       mbar_wait(&tfull[buf], (it >> 1) & 1);
       tc_fence_after_sync();
-      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + buf * (MAX_SUB * TILE_N);
+      const uint32_t taddr = tmem + ((uint32_t)(q * 32) << 16) + buf * UNIT_N;
       for (int sb = 0; sb < nsub; ++sb) {
         const int col0 = u->col0[sb], NT = u->nt[sb];
         float *yr = ybase + (size_t)u->det[sb] * c.ydet_stride;
@@ -400,7 +422,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
         const int nvalid = min(NT, ncols - col0);                 // columns of this sub-tile that exist
         for (int cc = grp * 32; cc < nvalid; cc += 64) {
           uint32_t v[32];
-          tmem_ld_32x32(taddr + sb * TILE_N + cc, v);
+          tmem_ld_32x32(taddr + u->tcol[sb] + cc, v);
           tmem_ld_wait();
           int slot = slot0 + cc;
           if (slot >= ylen) slot -= ylen;
@@ -569,13 +591,18 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
         for (size_t s0 = 0; s0 < subs.size();) {
           TcCorrUnit u; memset(&u, 0, sizeof(u));
           u.cls = (int)ci; u.row0 = r0; u.k0 = k0; u.k1 = k1; u.seg = sg;
-          // one wide sub-tile, or two narrow ones, per unit (256 accumulator columns)
-          u.nsub = (subs[s0].w > TILE_N || s0 + 1 >= subs.size() || subs[s0 + 1].w > TILE_N) ? 1 : 2;
-          for (int i = 0; i < u.nsub; ++i) {
-            u.det[i] = subs[s0 + i].det; u.col0[i] = subs[s0 + i].c0; u.nt[i] = (subs[s0 + i].w + 15) & ~15;
+          // pack up to MAX_SUB sub-tiles into the unit's UNIT_N accumulator columns (they share every U tile)
+          int cols = 0, xo = 0;
+          while (s0 < subs.size() && u.nsub < MAX_SUB) {
+            const int nt = (subs[s0].w + 15) & ~15;
+            if (cols + nt > UNIT_N) break;
+            const int i = u.nsub++;
+            u.det[i] = subs[s0].det; u.col0[i] = subs[s0].c0; u.nt[i] = nt;
+            u.tcol[i] = cols; u.soff[i] = 16 * (cols + i * KS); u.xoff[i] = xo;
+            cols += nt; xo += nt + (k1 - k0) + 8;
+            ++s0;
           }
           cu.push_back(u);
-          s0 += u.nsub;
         }
       }
   }
@@ -607,14 +634,14 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
   std::vector<int> cbegin, rbegin;
-  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
+  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1] + u.nt[2] + u.nt[3]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
   lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * ((rb[t.bank].Kpad + BK - 1) / BK + 1); }, rbegin);
   if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   const int rstages = planes == 2 ? 2 : 4;
   p->recon_smem = rstages * 3 * planes * TILE_BYTES + 1024 + 256;
-  p->corr_smem = (planes == 2 ? 4 : 6) * planes * TILE_BYTES + 2 * MAX_SUB * planes * STRIP_BYTES + MAX_SUB * XWIN * 4 + 1024 + 256;
+  p->corr_smem = (planes == 2 ? 4 : 6) * planes * TILE_BYTES + 2 * planes * STRIP_PLANE + XWIN_TOTAL * 4 + 1024 + 256;
   cudaError_t e;
   if (planes == 2) {
     e = cudaFuncSetAttribute(recon_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
