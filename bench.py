@@ -324,6 +324,18 @@ def run_ours(args):
         t_e2e += time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e, dev, world)
 
+    # ---- "empty push": the same five-kernel launch sequence on a one-template, 64-tap bank = launch overhead per push
+    from workloads import random_bank
+    tiny = lib.LloidStream([random_bank(1, 1, [(f0, 64, 1)], f0=f0).as_f32()], c.n_det, B, precision=PREC[args.precision],
+                           device=f"cuda:{local_rank}")
+    e0 = [torch.cuda.Event(enable_timing=True) for _ in range(40)]
+    e1 = [torch.cuda.Event(enable_timing=True) for _ in range(40)]
+    for i in range(40):
+        e0[i].record(); tiny.push_device(pool[i % n_total]); e1[i].record()
+    torch.cuda.synchronize()
+    empty_ms = float(np.median([a.elapsed_time(b) for a, b in zip(e0[8:], e1[8:])]))
+    tiny.close()
+
     # ---- per-stage device times (CUDA events recorded by the library on its stream) for the roofline
     st.set_stage_timing(True)
     for i in range(K):
@@ -337,7 +349,7 @@ def run_ours(args):
             dist.destroy_process_group()
         return
     line = assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
-                    l2_note, host_ms)
+                    l2_note, host_ms, empty_ms)
     if not args.no_cpu_baseline and world == 1 and banks:
         hist_s = 4
         strain_o = np.stack([make_strain(c.seed(det), (hist_s + 1) * f0) for det in range(c.n_det)])[:, :hist_s * f0 + B]
@@ -357,7 +369,7 @@ def measured_peaks():
 
 
 def assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
-             l2_note, host_ms):
+             l2_note, host_ms, empty_ms):
     peaks, peak_src = measured_peaks()
     value = whole_job_value(world, units_per_step, K, t_dev)
     e2e = whole_job_value(world, units_per_step, K, t_e2e)
@@ -414,8 +426,8 @@ def assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e
         "gpu_launches": launches * K, "wall_ms_timed_region": 1e3 * wall, "ms_step_min_med_max": [min(ms), float(np.median(ms)), max(ms)],
         "latency_ms": {"device_p50": float(np.percentile(ms, 50)), "device_p99": float(np.percentile(ms, 99)),
                        "device_max": max(ms), "host_launch_p50": float(np.percentile(host_ms, 50)),
-                       "host_launch_p99": float(np.percentile(host_ms, 99)),
-                       "note": "per-push device time (CUDA events around one lloid_stream_push) and host time of the call"},
+                       "host_launch_p99": float(np.percentile(host_ms, 99)), "empty_push_device_p50": empty_ms,
+                       "note": "per-push device time (CUDA events around one lloid_stream_push), host time of the call, and the device time of a push on a one-template 64-tap bank (launch overhead of the five-kernel sequence)"},
         "clocks": clocks, "roofline": roof,
     }
 
