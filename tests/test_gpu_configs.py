@@ -176,3 +176,44 @@ def test_config2_full_size_bench_configuration_sampled():
             assert np.all(same | (np.abs(p32[np.arange(bank.M), pk["sample"]] - p32[np.arange(bank.M), k]) <= 1e-6 * p32.max()))
             assert np.abs(pk["snr"] - np.sqrt(p32[np.arange(bank.M), pk["sample"]])).max() <= 1e-5 * np.sqrt(p32.max())
         print(f"full config 2 bank {bi}: sampled max err {err:.2e}, peak/sample agreement {np.mean(same):.4f}")
+
+
+def test_config3_twelve_banks_merged_classes_sampled():
+    """The first 12 banks of config 3 with their REAL slice layouts (rates, taps, delays from each bank's own chirp masses,
+    as bench.py's stand-ins) and 1000 templates each, 3 detectors: many slices of different banks share merged geometry
+    classes with per-member column offsets.  Basis counts are those bench.py measured for bank 0 (10, 12, 22, 44, 34, 52,
+    45, 39); U is random orthonormal, R random (generation stays within seconds).  Sampled templates of three banks vs
+    the oracle."""
+    _cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import lloid_snr
+    from workloads import CONFIGS, make_strain, random_bank
+    c = CONFIGS[3]
+    mcs = c.mchirps()
+    Ls = [10, 12, 22, 44, 34, 52, 45, 39]
+    banks = []
+    for b in range(12):
+        T, lay = c.layout(b, mcs)
+        shape = [(rate, (e - s0) // (c.f0 // rate), Ls[min(i, len(Ls) - 1)]) for i, (rate, s0, e) in enumerate(lay)]
+        banks.append(random_bank(c.seed(b), c.M, shape, f0=c.f0).as_f32())
+    assert len({(s.rate, s.n_taps, s.delay) for bk in banks for s in bk.slices}) > 20      # the layouts do differ
+    B, n_push = c.buffer_len, 3
+    strain = np.stack([make_strain(c.seed(det) + 7, n_push * B) for det in range(c.n_det)])
+    rng = np.random.default_rng(3333)
+    for bi in (0, 5, 11):
+        bank = banks[bi]
+        st = lib.LloidStream(banks, c.n_det, B, precision=lib.LLOID_PREC_F16_SPLIT)
+        for p in range(n_push):
+            peaks, rho = st.push(strain[:, p * B:(p + 1) * B], want_snr_bank=bi)
+        st.close()
+        tmpl = np.sort(rng.choice(bank.M, 8, replace=False))
+        rows = np.stack([2 * tmpl, 2 * tmpl + 1], axis=1).ravel()
+        worst = 0.0
+        for det in range(c.n_det):
+            ref = lloid_snr(bank, strain[det], (n_push - 1) * B, n_push * B, rows=list(rows))
+            z_ref = ref[0::2] + 1j * ref[1::2]
+            z = rho[det][2 * tmpl] + 1j * rho[det][2 * tmpl + 1]
+            rms = math.sqrt(np.mean(np.abs(z_ref) ** 2))
+            worst = max(worst, np.abs(z - z_ref).max() / rms)
+        print(f"config 3 (12 banks) bank {bi} [{bank.describe()[:48]}...]: sampled max err {worst:.2e}")
+        assert worst <= TOL[2]
