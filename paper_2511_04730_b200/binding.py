@@ -197,7 +197,7 @@ class LloidStream:
     """Owns bank and stream handles plus the torch device buffers a push needs."""
 
     def __init__(self, banks, n_detectors: int, buffer_len: int, precision: int = LLOID_PREC_F16_SPLIT,
-                 threshold: float = 0.0, device: str = "cuda:0"):
+                 threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("LloidStream needs a CUDA device (no CPU fallback)")
@@ -208,7 +208,7 @@ class LloidStream:
         self.Ms, self.bank_handles = [], []
         for b in banks:                      # any iterable: a generator lets the caller build banks one at a time
             self.Ms.append(b.M)
-            self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold))
+            self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down))
         self.cuda_stream = torch.cuda.current_stream(self.device)
         self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
         self.Mtot = lloid_stream_total_templates(self.handle)

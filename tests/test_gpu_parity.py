@@ -226,3 +226,23 @@ def test_large_decimation_and_single_big_upsample_stage(precision):
         print(f"D=128 bank det {det} precision {precision}: max err {emax:.3e}")
         assert emax <= TOL[precision]
         check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0))
+
+
+def test_n_down_option():
+    """lloid_options.n_down (PAPER.md:132 'typically set to 32'): a shorter decimator (n_down = 12) against the oracle
+    run with the same half length."""
+    _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import lloid_snr
+    from workloads import make_strain, random_bank
+    bank = random_bank(51, 18, [(2048, 512, 9), (512, 384, 13), (128, 96, 7)]).as_f32()
+    B, n_push = 512, 6
+    strain = np.stack([make_strain(510, B * n_push)])
+    st = lib.LloidStream([bank], 1, B, precision=lib.LLOID_PREC_F16_SPLIT, n_down=12)
+    rho = np.concatenate([st.push(strain[:, p * B:(p + 1) * B], want_snr_bank=0)[1] for p in range(n_push)], axis=2)
+    st.close()
+    ref = lloid_snr(bank, strain[0], n_down=12)
+    emax, _ = check_snr(rho[0], ref, TOL[2])
+    assert emax <= TOL[2]
+    ref32 = lloid_snr(bank, strain[0])
+    assert check_snr(rho[0], ref32, TOL[2])[0] > 10 * TOL[2]        # and it is NOT the n_down = 32 result
