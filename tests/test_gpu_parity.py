@@ -246,3 +246,21 @@ def test_n_down_option():
     assert emax <= TOL[2]
     ref32 = lloid_snr(bank, strain[0])
     assert check_snr(rho[0], ref32, TOL[2])[0] > 10 * TOL[2]        # and it is NOT the n_down = 32 result
+
+
+@pytest.mark.parametrize("precision", [2, 0])
+def test_degenerate_sizes(precision):
+    """One full-rate slice, 3 templates, 5 basis filters, buffers of 100 samples (not a multiple of any tile size),
+    3 detectors -- the smallest shapes the boundary accepts."""
+    _torch_cuda()
+    from oracle import lloid_snr
+    from workloads import make_strain, random_bank
+    bank = random_bank(61, 3, [(2048, 70, 5)]).as_f32()
+    B, n_push = 100, 7
+    strain = np.stack([make_strain(610 + d, B * n_push) for d in range(3)])
+    rho_gpu, peaks = run_gpu([bank], strain, B, precision)
+    for det in range(3):
+        ref = lloid_snr(bank, strain[det])
+        emax, _ = check_snr(rho_gpu[det], ref, TOL[precision])
+        assert emax <= TOL[precision]
+        check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0))
