@@ -85,7 +85,7 @@ struct UpRow {                       // one basis row of one slice of one bank: 
   void *yup;                         // bank's upsampled-Y array (plane 0)
   long long dst0;                    // element offset of (detector 0, sample 0, this row's column)
   long long yup_det_stride, yup_plane_stride;
-  int nseg, ypitch, kpitch, pad_;
+  int nseg, ypitch, kpitch, bank;    // bank: index of the owning bank (items are ordered by it for L2 locality)
 };
 struct UpItem {                      // <= 32 rows (lanes) that share one upsample chain: (rate, stage factors)
   int row0, nl;                      // rows [row0, row0 + nl) of the UpRow table
