@@ -1,12 +1,17 @@
 #!/usr/bin/env python
-"""bench.py -- LLOID hot-path throughput on B200 (driver contract).
+"""bench.py -- LLOID hot-path throughput and latency on B200 (driver contract).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config 2] [--precision split]
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference] [--config N] [--precision split]
 
-A STEP is one lloid_stream_push of one buffer (config 2: 1 s = 2048 samples) of every detector against every
-bank: a1 decimate -> a2 basis correlation -> a4 upsample -> a3 reconstruction -> a5 peaks.  The metric is
-BASELINE.json's: template*detector*data-seconds filtered per wall-second.  Workload = BASELINE.json configs[1]
-(4 SVD banks x 500 chirp templates, 2 detectors, 1 s buffers), seeded synthetic inputs from workloads/.
+A STEP is one lloid_stream_push of one buffer of every detector against every bank of the workload:
+a1 decimate -> a2 basis correlation -> a4 upsample -> a3 reconstruction -> a5 peaks.  The metric is BASELINE.json's:
+template*detector*data-seconds filtered per wall-second (plus per-buffer latency).
+
+With no --config the HEADLINE is the largest single-GPU workload, BASELINE.json configs[4] (full-scale: 1000 SVD banks x
+1000 templates, 3 detectors, 1 s buffers), and the same JSON line carries the records of configs[1], [2] and [3]
+(small-bank, mid-scale, low-latency 1/16 s buffers with p50/p99) under "other_configs".  `--config N` runs that config
+alone.  `--gpus N` (N > 1) re-executes itself under torch.distributed.run with N ranks unless it is already running
+under one; every rank filters an independent replica of the workload (weak scaling, no data-path collective).
 Prints ONE JSON line on rank 0.  `--impl reference` times the float64 CPU oracle (oracle/) on the host cores.
 """
 import argparse
@@ -27,87 +32,89 @@ METRIC = "template*detector*data-seconds filtered per wall-second"
 UNIT = "template*detector*data-s/s"
 PREC = {"ffma": 0, "f16": 1, "split": 2}
 PREC_DTYPE = {"ffma": "f32", "f16": "f16 operands, f32 accumulate", "split": "f16 hi+lo split operands (3 MMAs), f32 accumulate"}
+HEADLINE_CONFIG = 5                  # BASELINE.json configs[4]: the largest single-GPU workload
+NESTED_CONFIGS = (2, 3, 4)           # carried inside the headline line
 
 
-def parse():
+def parse(argv=None):
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--config", type=int, default=2, help="BASELINE.json config number (1-based); default 2 = configs[1]")
+    ap.add_argument("--config", type=int, default=0,
+                    help="BASELINE.json config number (1-based); default: headline config 5 with configs 2-4 nested")
     ap.add_argument("--precision", default=os.environ.get("LLOID_BENCH_PRECISION", "split"), choices=list(PREC))
     ap.add_argument("--banks", type=int, default=0, help="debug: use only the first n banks (0 = all; marks the run as reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-nested", action="store_true", help="headline config only")
     ap.add_argument("--no-flush", action="store_true", help="keep L2 warm between steps (reported in config)")
-    return ap.parse_args()
+    ap.add_argument("--plumbing-check", action="store_true",
+                    help="exercise launcher -> ranks -> process group -> max-over-ranks -> rank-0 line over gloo, no filtering (CPU test)")
+    return ap.parse_args(argv)
 
 
 # ---------------------------------------------------------------------------------------------------------
-# workload
+# workload: which banks are chirp-SVD banks, which are shape-faithful stand-ins
 # ---------------------------------------------------------------------------------------------------------
-N_REAL_BANKS = 4        # configs with many banks: this many real chirp-SVD banks, the rest shape-faithful stand-ins
+N_REAL_BANKS = 4        # evenly spaced chirp-SVD banks in the many-bank configs
+N_INJ_BANKS = 4         # plus the banks hit by the first injections of the parity stream (tests/test_gpu_fullsize.py)
 
 
-def _real_bank(args):
-    """One chirp-SVD bank of the config.  Generation is deterministic and slow for 1000-template banks (0.5-2 min),
-    so the result is memoised under /tmp (an input cache only: a miss just recomputes the same arrays)."""
-    cfg_no, b = args
-    import pickle
-    from workloads import CONFIGS
-    c = CONFIGS[cfg_no]
-    path = os.path.join("/tmp", "lloid_bank_cache", f"seed{c.seed(999)}_M{c.M}_nb{c.n_banks}_T{int(c.T_max)}_b{b}.pkl")
-    try:
-        with open(path, "rb") as f:
-            return b, pickle.load(f)
-    except Exception:
-        pass
-    bank = c.bank(b, method="gram" if c.M >= 1000 else "svd").as_f32()
-    try:
-        os.makedirs(os.path.dirname(path), exist_ok=True)
-        with open(path + f".{os.getpid()}", "wb") as f:
-            pickle.dump(bank, f, protocol=4)
-        os.replace(path + f".{os.getpid()}", path)
-    except Exception:
-        pass
-    return b, bank
+def parity_seconds(c):
+    """Length of the live-history parity stream of a config: the longest template plus 2 s."""
+    return int(c.T_max) + 2
 
 
-def bank_plan(cfg_no, n_banks_limit):
-    """(config, list of bank descriptions).  Configs 1-2: every bank is the config's chirp-SVD bank.  Configs 3-5
-    (100-1000 banks; one SVD bank takes 0.5-1 min of host time): N_REAL_BANKS evenly spaced real banks; every other
-    bank keeps its REAL slice layout (rates, taps, delays from its own chirp masses) and takes the basis counts L^s of
-    the nearest real bank, with seeded random orthonormal U and random R (SURVEY.md section 8d "scale handling")."""
+def real_bank_ids(c, nb):
+    """Banks built as real chirp-SVD banks: all of them for few-bank configs, else N_REAL_BANKS evenly spaced ones plus
+    the banks of the first N_INJ_BANKS distinct injected banks of the config's seeded parity-stream injections."""
+    if nb <= 8:
+        return list(range(nb))
+    ids = set(int(round(i * (nb - 1) / (N_REAL_BANKS - 1))) for i in range(N_REAL_BANKS))
+    extra = []
+    for inj in c.injections(parity_seconds(c)):
+        if inj.bank < nb and inj.bank not in ids and inj.bank not in extra:
+            extra.append(inj.bank)
+        if len(extra) >= N_INJ_BANKS:
+            break
+    return sorted(ids | set(extra))
+
+
+def bank_plan(cfg_no, n_banks_limit=0):
+    """(config, list of bank descriptions).  Every bank keeps its REAL slice layout (rates, taps, delays from its own
+    chirp masses); the banks of real_bank_ids are chirp-SVD banks, the others take the basis counts L^s of the nearest
+    real bank, with seeded random orthonormal U and random R (SURVEY.md section 8d "scale handling")."""
     from workloads import CONFIGS
     c = CONFIGS[cfg_no]
     nb = c.n_banks if not n_banks_limit else min(n_banks_limit, c.n_banks)
-    if nb <= 8:
-        return c, [("real", b) for b in range(nb)]
-    real = sorted(set(int(round(i * (nb - 1) / (N_REAL_BANKS - 1))) for i in range(N_REAL_BANKS)))
-    return c, [("real", b) if b in real else ("standin", b, min(real, key=lambda r: abs(r - b))) for b in range(nb)]
+    real = real_bank_ids(c, nb)
+    return c, [("real", b) if b in real else ("standin", b, min(real, key=lambda r: (abs(r - b), r))) for b in range(nb)]
 
 
-def iter_banks(cfg_no, plan, describe=None):
+def real_banks(cfg_no, ids, info=None):
+    """{bank index: chirp-SVD bank, float32-rounded}: workloads/bank_cache.py (parallel worker processes, .npz cache)."""
+    from workloads.bank_cache import real_banks as _rb
+    return _rb(cfg_no, ids, info)
+
+
+def standin_bank(c, b, like, mcs=None):
+    from workloads import random_bank
+    T, lay = c.layout(b, c.mchirps() if mcs is None else mcs)
+    Ls = [s.n_basis for s in like.slices]
+    shape = [(rate, (e - s0) // (c.f0 // rate), Ls[min(i, len(Ls) - 1)]) for i, (rate, s0, e) in enumerate(lay)]
+    return random_bank(c.seed(b), c.M, shape, f0=c.f0).as_f32()
+
+
+def iter_banks(cfg_no, plan, describe=None, info=None, real=None):
     """Yield the planned banks one at a time (the caller uploads each and drops it)."""
-    import multiprocessing as mp
-    from workloads import CONFIGS, random_bank
+    from workloads import CONFIGS
     c = CONFIGS[cfg_no]
     mcs = c.mchirps()
-    real_ids = [p[1] for p in plan if p[0] == "real"]
-    if len(real_ids) > 1 and c.M >= 1000:
-        with mp.get_context("fork").Pool(min(len(real_ids), os.cpu_count() or 1)) as pool:
-            real = dict(pool.map(_real_bank, [(cfg_no, b) for b in real_ids]))
-    else:
-        real = dict(_real_bank((cfg_no, b)) for b in real_ids)
+    if real is None:
+        real = real_banks(cfg_no, [p[1] for p in plan if p[0] == "real"], info)
     for p in plan:
-        if p[0] == "real":
-            bank = real[p[1]]
-        else:
-            _, b, src = p
-            T, lay = c.layout(b, mcs)
-            Ls = [s.n_basis for s in real[src].slices]
-            shape = [(rate, (e - s0) // (c.f0 // rate), Ls[min(i, len(Ls) - 1)]) for i, (rate, s0, e) in enumerate(lay)]
-            bank = random_bank(c.seed(b), c.M, shape, f0=c.f0).as_f32()
+        bank = real[p[1]] if p[0] == "real" else standin_bank(c, p[1], real[p[2]], mcs)
         if describe is not None:
             describe.append(("real " if p[0] == "real" else "standin ") + bank.describe())
         yield bank
@@ -126,6 +133,15 @@ def build_workload(cfg_no, n_banks_limit, seconds, rank=0, only_real=True):
     return c, banks, strain
 
 
+def config_dict(cfg_no, c, plan, reduced=False):
+    """The `config` object of the JSON line: names the WORKLOAD only, identical for both arms (--impl ours / reference)."""
+    n_real = sum(p[0] == "real" for p in plan)
+    return {"workload": f"BASELINE.json configs[{cfg_no - 1}] ({c.name})" + (" REDUCED (--banks)" if reduced else ""),
+            "n_banks": len(plan), "templates_per_bank": c.M, "n_detectors": c.n_det, "buffer_len": c.buffer_len,
+            "banks": (f"{n_real} chirp-SVD banks + {len(plan) - n_real} shape-faithful stand-ins (real slice layout, L^s of the "
+                      "nearest SVD bank, random orthonormal U / random R)")}
+
+
 def max_over_ranks(t_local, device, world):
     """Timed-region seconds of the slowest rank (all_reduce MAX over the job's process group)."""
     if world <= 1:
@@ -140,6 +156,13 @@ def max_over_ranks(t_local, device, world):
 def whole_job_value(world, units_per_step_per_rank, steps, seconds):
     """Aggregate throughput of `world` independent replicas (weak scaling, no data-path collective)."""
     return world * units_per_step_per_rank * steps / seconds
+
+
+def launcher_command(n, argv, port=None):
+    """The command `--gpus N` re-executes: one rank per GPU of this node under torch.distributed.run."""
+    port = port or os.environ.get("MASTER_PORT") or str(29500 + os.getpid() % 2000)
+    return [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", str(n), "--master-addr", "127.0.0.1",
+            "--master-port", str(port), os.path.abspath(__file__)] + list(argv)
 
 
 class ClockSampler:
@@ -199,13 +222,24 @@ def blas_threads():
         return os.cpu_count()
 
 
-def time_oracle(banks, strain, B, f0, budget_s, steps=1, warmup=0):
+def cpu_model():
+    try:
+        with open("/proc/cpuinfo") as f:
+            for line in f:
+                if line.lower().startswith("model name"):
+                    return line.split(":", 1)[1].strip()
+    except OSError:
+        pass
+    return "unknown"
+
+
+def time_oracle(banks, strain, B, f0, budget_s, steps=5, warmup=0, n_total_banks=None):
     """Time `steps` oracle steps on a bounded sample: as many leading banks as fit ~budget_s per step."""
     n_det = strain.shape[0]
     hist = strain.shape[1] - (steps + warmup) * B
     assert hist >= 0
     t0 = time.perf_counter()
-    oracle_step(banks[:1], strain, hist + B if hist + B <= strain.shape[1] else strain.shape[1], B)   # calibration
+    oracle_step(banks[:1], strain, hist + B, B)                                  # calibration (untimed)
     t1 = time.perf_counter() - t0
     nb = int(max(1, min(len(banks), budget_s / max(t1, 1e-3))))
     sub = banks[:nb]
@@ -216,57 +250,131 @@ def time_oracle(banks, strain, B, f0, budget_s, steps=1, warmup=0):
         oracle_step(sub, strain, hist + (warmup + s + 1) * B, B)
     dt = time.perf_counter() - t0
     units = sum(b.M for b in sub) * n_det * (B / f0) * steps
-    return units / dt, dt / steps, f"{nb} of {len(banks)} banks x {n_det} detectors x {steps} buffer(s) of {B} samples, float64 numpy"
+    n_all = n_total_banks if n_total_banks is not None else len(banks)
+    sample = (f"{nb} chirp-SVD bank(s) of the workload's {n_all} x {n_det} detectors x {steps} buffer(s) of {B} samples, float64 numpy"
+              + ("; EXTRAPOLATED linearly in banks to the whole workload (rate per template*detector*data-second)" if nb < n_all else ""))
+    return units / dt, dt / steps, sample
+
+
+def cpu_baseline_record(value, sample):
+    return {"value": value, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample,
+            "os_cpu_count": os.cpu_count(), "blas_threads": blas_threads(), "cpu_model": cpu_model()}
 
 
 def run_reference(args):
     """--impl reference: the oracle as it stands, on the host cores (rank 0 only)."""
     if int(os.environ.get("RANK", "0")) != 0:
         return
+    cfg_no = args.config or HEADLINE_CONFIG
     hist_s = 4
-    c, banks, strain = build_workload(args.config, args.banks, hist_s + args.steps + args.warmup)
+    c, plan = bank_plan(cfg_no, args.banks)
+    _, banks, strain = build_workload(cfg_no, args.banks, hist_s + -(-(args.steps + args.warmup) * c.buffer_len // c.f0))
     B = c.buffer_len
     budget = min(8.0, 200.0 / max(1, args.steps + args.warmup))
-    value, s_per_step, sample = time_oracle(banks, strain, B, c.f0, budget, args.steps, args.warmup)
+    strain = strain[:, :hist_s * c.f0 + (args.steps + args.warmup) * B]
+    value, s_per_step, sample = time_oracle(banks, strain, B, c.f0, budget, args.steps, args.warmup, len(plan))
     line = {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
             "warmup": args.warmup, "ms_per_step": 1e3 * s_per_step, "higher_is_better": True, "scaling": "weak",
             "vs_baseline": None, "dtype": "f64", "data": "synthetic",
-            "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({c.name})", "n_banks": len(banks),
-                       "templates_per_bank": c.M, "n_detectors": c.n_det, "buffer_len": B, "history_s": hist_s},
-            "cpu_baseline": {"value": value, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample},
+            "config": config_dict(cfg_no, c, plan, bool(args.banks) and args.banks < c.n_banks),
+            "run": {"history_s": hist_s, "note": "each step = one buffer of a bounded sample of the workload's chirp-SVD banks"},
+            "cpu_baseline": cpu_baseline_record(value, sample),
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
     print(json.dumps(line), flush=True)
 
 
-def run_ours(args):
-    import torch
-    import torch.distributed as dist
-    rank = int(os.environ.get("RANK", "0"))
-    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device -- the LLOID path has no CPU fallback")
-    torch.cuda.set_device(local_rank)
-    dev = torch.device("cuda", local_rank)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    import paper_2511_04730_b200 as lib
+# ---------------------------------------------------------------------------------------------------------
+# the CUDA arm
+# ---------------------------------------------------------------------------------------------------------
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        with open(p) as f:
+            return json.load(f), "measured (MEASURED_PEAKS.json)"
+    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
 
-    K, W = args.steps, args.warmup
-    n_total = 3 * K + W                        # device-timed K, end-to-end K, stage-timed K
-    from workloads import make_strain
-    c, plan = bank_plan(args.config, args.banks)
+
+def ncu_traffic(cfg_no, precision, stage):
+    """dram bytes per launch of a stage's kernel from the committed ncu captures (profiles/ncu_traffic.json), keyed by
+    (config, precision, stage); None when no capture of that config exists -- never another config's number."""
+    try:
+        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
+            return json.load(f).get(f"config{cfg_no}", {}).get(precision, {}).get(stage)
+    except (OSError, ValueError):
+        return None
+
+
+def roofline_record(cfg_no, precision, per_stage, work):
+    peaks, peak_src = measured_peaks()
+    dom = max(per_stage, key=per_stage.get)
+    dom_s = per_stage[dom] / 1e3
+    ffma = precision == "ffma"
+    # algorithmic work of the dominant kernel per launch (DESIGN.md "Kernels"): flop in the paper's order
+    algo = {"a2_correlate": work[2], "a3_reconstruct_a5_peaks": work[3], "a4_upsample_basis": work[4]}
+    executed = {"a2_correlate": work[0], "a3_reconstruct_a5_peaks": work[1]}
+    if dom in ("a2_correlate", "a3_reconstruct_a5_peaks"):
+        if ffma:
+            # dense contraction executed on the FP32 CUDA cores: peak = 148 SM x 128 FFMA lanes x 2 flop x max SM clock
+            peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
+            bound, peak_note = "alu", "148 SM x 128 lanes x 2 x sm_max_mhz (derived, DESIGN.md)"
+        else:
+            # fp16 and bf16 share one tcgen05 kind::f16 rate: nominal ratio 1.0 to the measured bf16 peak (sustained:
+            # the kernel is timed inside a long step)
+            peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+            bound, peak_note = "tensor", f"bf16_tflops_sustained x 1.0 (fp16 = bf16 rate), {peak_src}"
+        roof = {"bound": bound, "kernel": dom, "achieved": algo[dom] / dom_s / 1e12, "peak": peak, "unit": "TFLOP/s",
+                "frac": algo[dom] / dom_s / 1e12 / peak, "traffic": None,
+                "executed_tflops": executed[dom] / dom_s / 1e12, "executed_frac": executed[dom] / dom_s / 1e12 / peak,
+                "peak_source": peak_note}
+    else:
+        byt = work[6] if dom == "a4_upsample_basis" else 0.0
+        peak = float(peaks["hbm_gbs"])
+        roof = {"bound": "hbm", "kernel": dom, "achieved": byt / dom_s / 1e9, "peak": peak, "unit": "GB/s",
+                "frac": byt / dom_s / 1e9 / peak, "traffic": None, "peak_source": peak_src}
+    roof["traffic"] = ncu_traffic(cfg_no, precision, dom)
+    if roof["traffic"] is None:
+        roof["traffic_note"] = "no ncu --set full capture of this config/kernel at this commit (profiles/ncu_traffic.json)"
+    roof["ms_per_launch"] = per_stage[dom]
+    roof["stage_ms_per_push"] = per_stage
+    roof["stage_share"] = {k: v / max(sum(per_stage.values()), 1e-12) for k, v in per_stage.items()}
+    # every tensor/HBM stage against its own roofline (the dominant one is repeated above)
+    tpeak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
+    roof["per_stage"] = {}
+    for k in ("a2_correlate", "a3_reconstruct_a5_peaks"):
+        if per_stage.get(k, 0) > 0 and not ffma:
+            roof["per_stage"][k] = {"algorithmic_tflops": algo[k] / per_stage[k] / 1e9, "frac": algo[k] / per_stage[k] / 1e9 / tpeak,
+                                    "executed_frac": executed[k] / per_stage[k] / 1e9 / tpeak}
+    if per_stage.get("a4_upsample_basis", 0) > 0:
+        roof["per_stage"]["a4_upsample_basis"] = {"gbs_on_intermediate_bytes": work[6] / per_stage["a4_upsample_basis"] / 1e6,
+                                                  "frac_of_hbm": work[6] / per_stage["a4_upsample_basis"] / 1e6 / float(peaks["hbm_gbs"])}
+    return roof
+
+
+def measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, K, W, precision, banks_limit, no_flush,
+                   shared=None, keep_real=False):
+    """Build the stream of one config and time it.  Returns (record, kept) where kept = dict(handles, Ms, real banks) so
+    a config with the same banks (config 4 = config 3 at another buffer length) can reuse the uploaded banks."""
+    from workloads import make_strain, random_bank
+    c, plan = bank_plan(cfg_no, banks_limit)
     B, f0 = c.buffer_len, c.f0
-    descr = []
-    keep = []                                  # banks kept on the host only when the oracle baseline needs them
-    def gen():
-        for bank in iter_banks(args.config, plan, descr):
-            if descr[-1].startswith("real"):
-                keep.append(bank)
-            yield bank
-    st = lib.LloidStream(gen(), c.n_det, B, precision=PREC[args.precision], device=f"cuda:{local_rank}")
-    banks = keep
+    info = {}
+    t_build0 = time.perf_counter()
+    if shared is not None:
+        st = lib.LloidStream(None, c.n_det, B, precision=PREC[precision], device=f"cuda:{local_rank}",
+                             bank_handles=shared["handles"], Ms=shared["Ms"])
+        descr, keep = shared["descr"], shared["real"]
+    else:
+        descr, keep = [], []
+
+        def gen():
+            for bank in iter_banks(cfg_no, plan, descr, info):
+                if descr[-1].startswith("real") and keep_real:
+                    keep.append(bank)
+                yield bank
+        st = lib.LloidStream(gen(), c.n_det, B, precision=PREC[precision], device=f"cuda:{local_rank}")
+    build_s = time.perf_counter() - t_build0
+    n_total = 3 * K + W                        # device-timed K, end-to-end K, stage-timed K
     n_seconds = -(-n_total * B // f0)
     strain = np.stack([make_strain(c.seed(det) + 100 * rank, n_seconds * f0) for det in range(c.n_det)])[:, :n_total * B]
     units_per_step = st.Mtot * c.n_det * (B / f0)
@@ -275,10 +383,10 @@ def run_ours(args):
     # L2 policy: the operands (U, R) and intermediates one push touches either exceed the 126 MB L2 several times
     # over (configs 3-5) or the L2 is flushed between steps by writing 256 MiB (configs 1-2)
     touched = work[5] + work[6] / 2
-    do_flush = (not args.no_flush) and touched < 4 * 126e6
+    do_flush = (not no_flush) and touched < 4 * 126e6
     flush_buf = torch.empty(256 << 20, dtype=torch.uint8, device=dev) if do_flush else None
     l2_note = ("flushed between steps (256 MiB memset, untimed)" if do_flush else
-               ("warm (--no-flush)" if args.no_flush and touched < 4 * 126e6 else
+               ("warm (--no-flush)" if no_flush and touched < 4 * 126e6 else
                 f"not flushed: one push touches {touched / 1e6:.0f} MB of operands/intermediates (> 4x the 126 MB L2)"))
 
     def flush():
@@ -324,9 +432,8 @@ def run_ours(args):
         t_e2e += time.perf_counter() - t0
     t_e2e = max_over_ranks(t_e2e, dev, world)
 
-    # ---- "empty push": the same five-kernel launch sequence on a one-template, 64-tap bank = launch overhead per push
-    from workloads import random_bank
-    tiny = lib.LloidStream([random_bank(1, 1, [(f0, 64, 1)], f0=f0).as_f32()], c.n_det, B, precision=PREC[args.precision],
+    # ---- "empty push": the same launch sequence on a one-template, 64-tap bank = launch overhead per push
+    tiny = lib.LloidStream([random_bank(1, 1, [(f0, 64, 1)], f0=f0).as_f32()], c.n_det, B, precision=PREC[precision],
                            device=f"cuda:{local_rank}")
     e0 = [torch.cuda.Event(enable_timing=True) for _ in range(40)]
     e1 = [torch.cuda.Event(enable_timing=True) for _ in range(40)]
@@ -343,98 +450,121 @@ def run_ours(args):
     n_cov, stage_ms = st.stage_times()
     st.set_stage_timing(False)
     launches = st.launches_per_push
+    d2h = int(st.peaks_host.numel() * st.peaks_host.element_size())
+    handles, Ms = st.release_banks() if shared is None else (None, None)      # the caller owns (and frees) the bank handles
     st.close()
-    if rank != 0:
-        if world > 1:
-            dist.destroy_process_group()
-        return
-    line = assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
-                    l2_note, host_ms, empty_ms)
-    if not args.no_cpu_baseline and world == 1 and banks:
-        hist_s = 4
-        strain_o = np.stack([make_strain(c.seed(det), (hist_s + 1) * f0) for det in range(c.n_det)])[:, :hist_s * f0 + B]
-        v, s_per, sample = time_oracle(banks, strain_o, B, f0, 15.0, 1, 0)
-        line["cpu_baseline"] = {"value": v, "unit": UNIT, "cores": blas_threads(), "kind": "oracle", "sample": sample}
-    print(json.dumps(line), flush=True)
+    del pool, flush_buf
+    torch.cuda.empty_cache()
+
+    per_stage = {k: v / max(n_cov, 1) for k, v in stage_ms.items()}            # ms per push
+    rec = {
+        "metric": METRIC, "value": whole_job_value(world, units_per_step, K, t_dev), "unit": UNIT, "n_gpus": world,
+        "steps": K, "warmup": W, "ms_per_step": 1e3 * t_dev / K, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": PREC_DTYPE[precision], "data": "synthetic",
+        "config": config_dict(cfg_no, c, plan, bool(banks_limit) and banks_limit < c.n_banks),
+        "run": {"slices": descr[:2] + descr[-2:], "precision": precision, "l2": l2_note,
+                "timing": "sum of per-step CUDA-event intervals (push only), max over ranks",
+                "multi_gpu": "independent replicas of the workload, no data-path collective",
+                "stream_build_s": build_s, "banks_shared_with": (shared or {}).get("cfg"), **info},
+        "e2e": {"value": whole_job_value(world, units_per_step, K, t_e2e), "unit": UNIT, "h2d_bytes_per_step": c.n_det * B * 4,
+                "d2h_bytes_per_step": d2h, "ms_per_step": 1e3 * t_e2e / K},
+        "gpu_launches": launches * K, "wall_ms_timed_region": 1e3 * wall,
+        "ms_step_min_med_max": [min(ms), float(np.median(ms)), max(ms)],
+        "latency_ms": {"device_p50": float(np.percentile(ms, 50)), "device_p99": float(np.percentile(ms, 99)),
+                       "device_max": max(ms), "host_launch_p50": float(np.percentile(host_ms, 50)),
+                       "host_launch_p99": float(np.percentile(host_ms, 99)), "empty_push_device_p50": empty_ms,
+                       "realtime_budget_ms": 1e3 * B / f0,
+                       "note": "per-push device time (CUDA events around one lloid_stream_push), host time of the call, and the "
+                               "device time of a push on a one-template 64-tap bank (launch overhead of the kernel sequence)"},
+        "clocks": clocks, "roofline": roofline_record(cfg_no, precision, per_stage, work),
+    }
+    kept = {"cfg": cfg_no, "handles": handles, "Ms": Ms, "descr": descr, "real": keep}
+    return rec, kept
+
+
+def free_kept(lib, kept):
+    for h in (kept or {}).get("handles") or []:
+        lib.lloid_bank_destroy(h)
+
+
+def run_plumbing_check(args):
+    """CPU-only: launcher -> ranks -> gloo process group -> barrier -> max over ranks -> one rank-0 line (no filtering)."""
+    import torch
+    import torch.distributed as dist
+    rank, world = int(os.environ.get("RANK", "0")), int(os.environ.get("WORLD_SIZE", "1"))
+    if world > 1:
+        dist.init_process_group("gloo")
+        dist.barrier()
+    t = max_over_ranks(0.010 * (rank + 1), torch.device("cpu"), world)       # the last rank is the slow one
+    if rank == 0:
+        print(json.dumps({"plumbing_check": True, "n_gpus": world, "gpus_arg": args.gpus, "t": t,
+                          "value": whole_job_value(world, 64.0, args.steps, t), "scaling": "weak"}), flush=True)
     if world > 1:
         dist.destroy_process_group()
 
 
-def measured_peaks():
-    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
-    if os.path.exists(p):
-        with open(p) as f:
-            return json.load(f), "measured (MEASURED_PEAKS.json)"
-    return {"hbm_gbs": 6650.0, "bf16_tflops": 1590.0, "bf16_tflops_sustained": 1400.0, "sm_max_mhz": 1965.0}, "fallback (B200_PROFILING.md)"
+def run_ours(args):
+    import torch
+    import torch.distributed as dist
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device -- the LLOID path has no CPU fallback")
+    torch.cuda.set_device(local_rank)
+    dev = torch.device("cuda", local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+    import paper_2511_04730_b200 as lib
 
-
-def assemble(args, c, descr, world, K, W, units_per_step, t_dev, ms, wall, t_e2e, stage_ms, n_cov, work, launches, clocks,
-             l2_note, host_ms, empty_ms):
-    peaks, peak_src = measured_peaks()
-    value = whole_job_value(world, units_per_step, K, t_dev)
-    e2e = whole_job_value(world, units_per_step, K, t_e2e)
-    per_stage = {k: v / max(n_cov, 1) for k, v in stage_ms.items()}            # ms per push
-    dom = max(per_stage, key=per_stage.get)
-    dom_s = per_stage[dom] / 1e3
-    ffma = args.precision == "ffma"
-    # algorithmic work of the dominant kernel per launch: flop in the paper's order
-    algo = {"a2_correlate": work[2], "a3_reconstruct_a5_peaks": work[3], "a4_upsample_basis": work[4]}
-    executed = {"a2_correlate": work[0], "a3_reconstruct_a5_peaks": work[1]}
-    if dom in ("a2_correlate", "a3_reconstruct_a5_peaks"):
-        if ffma:
-            # dense contraction executed on the FP32 CUDA cores: peak = 148 SM x 128 FFMA lanes x 2 flop x max SM clock
-            peak = 148 * 128 * 2 * peaks.get("sm_max_mhz", 1965.0) * 1e6 / 1e12
-            bound, peak_note = "alu", "148 SM x 128 lanes x 2 x sm_max_mhz (derived, DESIGN.md)"
-        else:
-            # fp16 and bf16 share one tcgen05 kind::f16 rate: nominal ratio 1.0 to the measured bf16 peak (sustained:
-            # the kernel is timed inside a long step)
-            peak = float(peaks.get("bf16_tflops_sustained", peaks["bf16_tflops"]))
-            bound, peak_note = "tensor", f"bf16_tflops_sustained x 1.0 (fp16 = bf16 rate), {peak_src}"
-        roof = {"bound": bound, "kernel": dom, "achieved": algo[dom] / dom_s / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "frac": algo[dom] / dom_s / 1e12 / peak, "traffic": None,
-                "executed_tflops": executed[dom] / dom_s / 1e12, "executed_frac": executed[dom] / dom_s / 1e12 / peak,
-                "peak_source": peak_note}
-    else:
-        byt = work[6] if dom == "a4_upsample_basis" else 0.0
-        peak = float(peaks["hbm_gbs"])
-        roof = {"bound": "hbm", "kernel": dom, "achieved": byt / dom_s / 1e9, "peak": peak, "unit": "GB/s",
-                "frac": byt / dom_s / 1e9 / peak, "traffic": None, "peak_source": peak_src}
-    try:
-        with open(os.path.join(ROOT, "profiles", "ncu_traffic.json")) as f:
-            roof["traffic"] = json.load(f).get(args.precision, {}).get(dom)
-    except OSError:
-        pass
-    roof["ms_per_launch"] = per_stage[dom]
-    roof["stage_ms_per_push"] = per_stage
-    roof["stage_share"] = {k: v / max(sum(per_stage.values()), 1e-12) for k, v in per_stage.items()}
-    reduced = bool(args.banks) and args.banks < c.n_banks
-    banks = descr
-    return {
-        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": K, "warmup": W,
-        "ms_per_step": 1e3 * t_dev / K, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": PREC_DTYPE[args.precision], "data": "synthetic",
-        "config": {"workload": f"BASELINE.json configs[{args.config - 1}] ({c.name})" + (" REDUCED (--banks)" if reduced else ""),
-                   "n_banks": len(descr), "templates_per_bank": c.M, "n_detectors": c.n_det, "buffer_len": c.buffer_len,
-                   "banks": (f"{sum(d.startswith('real') for d in descr)} chirp-SVD banks + "
-                             f"{sum(d.startswith('standin') for d in descr)} shape-faithful stand-ins (real slice layout, L^s of the "
-                             "nearest SVD bank, random orthonormal U / random R)"),
-                   "slices": descr[:2] + descr[-2:], "precision": args.precision, "l2": l2_note,
-                   "timing": "sum of per-step CUDA-event intervals (push only), max over ranks",
-                   "multi_gpu": "independent replicas of the workload, no data-path collective"},
-        "e2e": {"value": e2e, "unit": UNIT, "h2d_bytes_per_step": c.n_det * c.buffer_len * 4,
-                "d2h_bytes_per_step": int(c.n_det * len(descr) * c.M * 12), "ms_per_step": 1e3 * t_e2e / K},
-        "gpu_launches": launches * K, "wall_ms_timed_region": 1e3 * wall, "ms_step_min_med_max": [min(ms), float(np.median(ms)), max(ms)],
-        "latency_ms": {"device_p50": float(np.percentile(ms, 50)), "device_p99": float(np.percentile(ms, 99)),
-                       "device_max": max(ms), "host_launch_p50": float(np.percentile(host_ms, 50)),
-                       "host_launch_p99": float(np.percentile(host_ms, 99)), "empty_push_device_p50": empty_ms,
-                       "note": "per-push device time (CUDA events around one lloid_stream_push), host time of the call, and the device time of a push on a one-template 64-tap bank (launch overhead of the five-kernel sequence)"},
-        "clocks": clocks, "roofline": roof,
-    }
+    K, W = args.steps, args.warmup
+    head_cfg = args.config or HEADLINE_CONFIG
+    want_oracle = not args.no_cpu_baseline and world == 1
+    line, kept = measure_config(lib, torch, dist, dev, local_rank, rank, world, head_cfg, K, W, args.precision, args.banks,
+                                args.no_flush, keep_real=want_oracle)
+    real_head = kept["real"]
+    free_kept(lib, kept)
+    if not args.config and not args.no_nested:
+        others, kept3 = {}, None
+        for cfg_no in NESTED_CONFIGS:
+            k_cfg = max(K, 200) if cfg_no == 4 else K                         # p99 of the 1/16 s pushes needs >= 200 samples
+            shared = kept3 if cfg_no == 4 and kept3 and kept3.get("handles") else None
+            rec, kept_n = measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, k_cfg, W, args.precision, 0,
+                                         args.no_flush, shared=shared, keep_real=(cfg_no == 3))
+            others[f"config{cfg_no}"] = rec
+            if cfg_no == 3:
+                kept3 = kept_n
+            elif shared is None:
+                free_kept(lib, kept_n)
+        free_kept(lib, kept3)
+        line["other_configs"] = others
+    if rank == 0:
+        if want_oracle and real_head:
+            from workloads import CONFIGS, make_strain
+            c = CONFIGS[head_cfg]
+            hist_s, n_buf = 4, 5
+            n = hist_s * c.f0 + n_buf * c.buffer_len
+            strain_o = np.stack([make_strain(c.seed(det), -(-n // c.f0) * c.f0) for det in range(c.n_det)])[:, :n]
+            v, _, sample = time_oracle(real_head, strain_o, c.buffer_len, c.f0, 4.0, n_buf, 0, line["config"]["n_banks"])
+            line["cpu_baseline"] = cpu_baseline_record(v, sample)
+        print(json.dumps(line), flush=True)
+    if world > 1:
+        dist.destroy_process_group()
 
 
 def main():
     args = parse()
-    if args.impl == "reference":
+    env_world = os.environ.get("WORLD_SIZE")
+    if args.gpus > 1 and env_world is None:
+        # not yet under a launcher: start one rank per GPU (the driver's own torchrun command lands in the branch below)
+        cmd = launcher_command(args.gpus, sys.argv[1:])
+        os.execv(cmd[0], cmd)
+    if env_world is not None and int(env_world) != args.gpus:
+        raise SystemExit(f"bench.py: --gpus {args.gpus} but the launcher started WORLD_SIZE={env_world} ranks; "
+                         f"run `python bench.py --gpus N` (it launches torch.distributed.run itself) or give both the same N")
+    if args.plumbing_check:
+        run_plumbing_check(args)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         run_ours(args)

@@ -13,8 +13,10 @@
  * SNR sample k of a push is stream sample n0+k (n0 = samples pushed before); it reads strain <= n0+k only.
  *
  * All pointers are plain host or device pointers as stated per argument; no C++/torch types cross this
- * boundary.  Every function returns 0 (LLOID_OK) or a negative lloid_status; on failure nothing is changed
- * and lloid_last_error() (thread-local) describes the reason.  There is no CPU fallback: every call that
+ * boundary.  Every function returns 0 (LLOID_OK) or a negative lloid_status and lloid_last_error()
+ * (thread-local) describes the reason.  Argument/state errors (EINVAL, ELATENCY, ESTATE, ENOMEM) change nothing.
+ * LLOID_ECUDA from lloid_stream_push means a kernel launch failed part-way: the stream's device state is then
+ * inconsistent and every further push returns LLOID_ESTATE until lloid_state_reset.  There is no CPU fallback: every call that
  * computes needs a CUDA device of compute capability 10.0 (sm_100a).
  */
 #ifndef LLOID_H_
@@ -34,7 +36,7 @@ typedef enum {
                           upsample chain: delay_s < n_down + H_g (PAPER.md:161-163 causality condition) */
   LLOID_ENOMEM = -3,   /* host or device allocation failed */
   LLOID_ECUDA = -4,    /* a CUDA runtime/driver call failed, or the device is not sm_100 */
-  LLOID_ESTATE = -5    /* call not valid in this state (e.g. debug_bank out of range) */
+  LLOID_ESTATE = -5    /* call not valid in this state (debug_bank out of range; push after a failed push) */
 } lloid_status;
 
 typedef enum {
@@ -85,7 +87,7 @@ void lloid_bank_destroy(lloid_bank *bank);
  * detectors: flat-PSD synthetic case; per-detector banks = one stream per detector).
  * buffer_len (f0 samples per push) must be a multiple of every bank's largest decimation factor.
  * cuda_stream is a cudaStream_t (NULL = legacy default stream); all work of push/reset is enqueued on it.
- * All banks must use the same precision and must outlive the stream. */
+ * All banks must use the same precision, n_down and threshold (EINVAL otherwise) and must outlive the stream. */
 int lloid_stream_create(lloid_stream **out, const lloid_bank *const *banks, int32_t n_banks,
                         int32_t n_detectors, int32_t buffer_len, void *cuda_stream);
 void lloid_stream_destroy(lloid_stream *stream);

@@ -197,7 +197,9 @@ class LloidStream:
     """Owns bank and stream handles plus the torch device buffers a push needs."""
 
     def __init__(self, banks, n_detectors: int, buffer_len: int, precision: int = LLOID_PREC_F16_SPLIT,
-                 threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32):
+                 threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32, bank_handles=None, Ms=None):
+        """banks: iterable of Bank-like objects (uploaded here, owned by this object), or None with `bank_handles`
+        (+ their template counts `Ms`): existing lloid_bank handles owned by the caller (several streams can share them)."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("LloidStream needs a CUDA device (no CPU fallback)")
@@ -206,9 +208,13 @@ class LloidStream:
         torch.cuda.set_device(self.device)
         self.n_det, self.B = n_detectors, buffer_len
         self.Ms, self.bank_handles = [], []
-        for b in banks:                      # any iterable: a generator lets the caller build banks one at a time
-            self.Ms.append(b.M)
-            self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down))
+        self.owns_banks = bank_handles is None
+        if bank_handles is not None:
+            self.bank_handles, self.Ms = list(bank_handles), list(Ms)
+        else:
+            for b in banks:                  # any iterable: a generator lets the caller build banks one at a time
+                self.Ms.append(b.M)
+                self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down))
         self.cuda_stream = torch.cuda.current_stream(self.device)
         self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
         self.Mtot = lloid_stream_total_templates(self.handle)
@@ -258,12 +264,18 @@ class LloidStream:
     def launches_per_push(self) -> int:
         return lloid_stream_launches_per_push(self.handle)
 
+    def release_banks(self):
+        """Hand the bank handles to the caller (who must lloid_bank_destroy them after every stream using them is closed)."""
+        self.owns_banks = False
+        return list(self.bank_handles), list(self.Ms)
+
     def close(self):
         if getattr(self, "handle", None):
             lloid_stream_destroy(self.handle)
             self.handle = None
-        for b in getattr(self, "bank_handles", []):
-            lloid_bank_destroy(b)
+        if getattr(self, "owns_banks", False):
+            for b in getattr(self, "bank_handles", []):
+                lloid_bank_destroy(b)
         self.bank_handles = []
 
     def __del__(self):

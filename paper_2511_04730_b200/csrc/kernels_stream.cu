@@ -60,7 +60,7 @@ __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, cons
   const int ring_base = (int)(((n0 % rlen0) + rlen0) % rlen0);   // ring slot of stream sample n0
   auto strain_at = [&](long long idx) {
     const long long rel = idx - n0;
-    if (rel >= 0) return sd[rel];
+    if (rel >= 0) return rel < P.B ? sd[rel] : 0.f;       // beyond the pushed buffer: outputs that do not exist (discarded)
     if (idx < 0) return 0.f;
     long long sl = ring_base + rel;                        // rel in (-rlen0, 0): one wrap at most
     if (sl < 0) sl += rlen0;
@@ -77,7 +77,7 @@ __global__ void __launch_bounds__(256) decimate_kernel(const DecimParams P, cons
   for (int i = threadIdx.x; i < nwin; i += 256) {
     const long long idx = base + i, rel = idx - n0;
     float v;
-    if (rel >= 0) v = sd[rel];
+    if (rel >= 0) v = rel < P.B ? sd[rel] : 0.f;            // never read past the caller's [n_det][B] buffer
     else if (idx < 0) v = 0.f;
     else {
       long long sl = ring_base + rel;                      // rel in (-rlen0, 0): one wrap at most
@@ -132,7 +132,6 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   lane = basis row (of any slice / bank with that chain: UpRow gives its source ring row and destination column).
 // ------------------------------------------------------------------------------------------------
 #define UP_RUN 8
-struct UpTaps2 { float t[16]; };   // g_2[2k+1], k = 0..15: the 16 non-zero taps of the x2 interpolation phase (Eq. 7)
 #define UP_CHUNK 512  // f0 samples per CTA
 #define UP_MAXW (UP_CHUNK / 2 + 40)   // widest staged level: chunk/2 + 2*8 + 1 (+ slack)
 template <int HALF_PLANES>
@@ -340,26 +339,24 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
   }
 }
 
+// Per-device kernel attributes (dynamic shared memory opt-in) and the x2 taps: called by every lloid_stream_create on
+// its current device (the attribute is per device/context, not per process).
+cudaError_t upsample_configure(UpTaps2 *t2) {
+  const int smem = 2 * UP_MAXW * 32 * (int)sizeof(float);
+  cudaError_t e = cudaFuncSetAttribute(upsample_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(upsample_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  if (e == cudaSuccess) e = cudaFuncSetAttribute(upsample_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
+  for (int k = 0; k < 16; ++k) {                         // Eq. 4 with f = 2, c = 16 (same float64 -> fp32 values as uptaps)
+    const double x = (2 * k + 1) - 16.0, a = M_PI * x / 2.0, b = M_PI * x / 16.0;
+    t2->t[k] = (float)((sin(a) / a) * (sin(b) / b));
+  }
+  return e;
+}
+
 cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
-                            const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st) {
+                            const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
   const int smem = 2 * UP_MAXW * 32 * (int)sizeof(float);
-  static bool attr = false;
-  if (!attr) {
-    cudaFuncSetAttribute(upsample_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(upsample_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    cudaFuncSetAttribute(upsample_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
-    attr = true;
-  }
-  static UpTaps2 t2;                                     // Eq. 4 with f = 2, c = 16 (same float64 -> fp32 values as uptaps)
-  static bool have = false;
-  if (!have) {
-    for (int k = 0; k < 16; ++k) {
-      const double x = (2 * k + 1) - 16.0, a = M_PI * x / 2.0, b = M_PI * x / 16.0;
-      t2.t[k] = (float)((sin(a) / a) * (sin(b) / b));
-    }
-    have = true;
-  }
   if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   else upsample_kernel<2><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);

@@ -95,6 +95,10 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
       else {
         const GroupInfo &p = b->groups.back();
         g.f = g.D / p.D;
+        if (g.f > (1 << LLOID_MAX_GROUPS)) {              // the upsampler's tap table covers stage factors up to 2^LLOID_MAX_GROUPS
+          set_error("bank_create: slice %d: upsample stage factor %d exceeds %d", s, g.f, 1 << LLOID_MAX_GROUPS);
+          delete b; return LLOID_EINVAL;
+        }
         g.A = (p.A + g.f - 1) / g.f + LLOID_NUP;
         g.H = (int)floor_div(p.H - 1, g.f) + LLOID_NUP + 1;
       }

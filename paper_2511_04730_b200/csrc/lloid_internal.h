@@ -108,8 +108,10 @@ struct PeakPartial { float p; int idx; float re, im; };
 cudaError_t launch_decimate(const DecimParams &P, const float *strain, const long long *n0, cudaStream_t st);
 cudaError_t launch_corr_ffma(const CorrClass *cls_dev, const CorrTile *tiles_dev, int n_tiles, int n_det,
                              const long long *n0, cudaStream_t st);
+struct UpTaps2 { float t[16]; };     // g_2[2k+1], k = 0..15: the 16 non-zero taps of the x2 interpolation phase (Eq. 7)
+cudaError_t upsample_configure(UpTaps2 *t2);
 cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
-                            const int *uptap_off, const long long *n0, int out_half_planes, cudaStream_t st);
+                            const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st);
 cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,

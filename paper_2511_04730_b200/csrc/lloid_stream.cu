@@ -32,6 +32,8 @@ struct lloid_stream {
   std::vector<void *> allocs;                      // every cudaMalloc of this stream
   std::vector<std::pair<void *, size_t>> state;    // (ptr, bytes) zeroed by reset
   int up_planes, up_chunk;
+  UpTaps2 taps2;                                   // x2 interpolation taps (kernel parameter of the upsampler)
+  bool failed;                                     // a launch of an earlier push failed: state is inconsistent until reset
   double work[8];
   bool stage_timing;
   std::vector<cudaEvent_t> ev_pool;               // free events
@@ -95,8 +97,8 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   for (int b = 0; b < n_banks; ++b) {
     if (!banks[b]) { set_error("stream_create: bank %d is NULL", b); return LLOID_EINVAL; }
     if (banks[b]->f0 != banks[0]->f0 || banks[b]->opt.precision != banks[0]->opt.precision ||
-        banks[b]->opt.n_down != banks[0]->opt.n_down) {
-      set_error("stream_create: bank %d differs from bank 0 in strain rate, precision or n_down", b); return LLOID_EINVAL;
+        banks[b]->opt.n_down != banks[0]->opt.n_down || banks[b]->opt.threshold != banks[0]->opt.threshold) {
+      set_error("stream_create: bank %d differs from bank 0 in strain rate, precision, n_down or threshold", b); return LLOID_EINVAL;
     }
     for (const SliceInfo &si : banks[b]->slices) Dmax = std::max(Dmax, si.D);
   }
@@ -106,7 +108,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->banks.assign(banks, banks + n_banks);
   s->n_det = n_det; s->B = B; s->f0 = banks[0]->f0; s->precision = banks[0]->opt.precision;
   s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold;
-  s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false;
+  s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false; s->failed = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
   s->up_chunk = std::min(B, 512);                   // = UP_CHUNK of kernels_stream.cu
@@ -116,6 +118,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   CK(cudaGetDeviceProperties(&prop, dev));
   if (prop.major != 10) { set_error("stream_create: device %s is sm_%d%d, this library is sm_100a only", prop.name, prop.major, prop.minor); lloid_stream_destroy(s); return LLOID_ECUDA; }
   CK(dev_alloc(s, &s->n0_dev, 1, true));
+  CK(upsample_configure(&s->taps2));                  // per-device kernel attributes: set on every create
 
   // ---- rates and their rings
   std::map<int, long long> span;                       // D -> max(delay + N) over slices at that rate
@@ -345,6 +348,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
                                  int32_t debug_bank) {
   if (!s || !strain || !peaks) { set_error("stream_push: stream, strain and peaks must be non-NULL"); return LLOID_EINVAL; }
   if (snr_debug && (debug_bank < 0 || debug_bank >= (int)s->banks.size())) { set_error("stream_push: debug_bank %d out of range", debug_bank); return LLOID_ESTATE; }
+  if (s->failed) { set_error("stream_push: an earlier push failed part-way; call lloid_state_reset first"); return LLOID_ESTATE; }
   std::vector<cudaEvent_t> ev;
   if (s->stage_timing) {
     for (int i = 0; i <= LLOID_N_STAGES; ++i) {
@@ -365,7 +369,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   mark(2);
   if (e == cudaSuccess)
     e = launch_upsample(s->items_dev, s->uprows_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
-                        s->n0_dev, s->up_planes, s->st);
+                        s->n0_dev, s->up_planes, s->taps2, s->st);
   mark(3);
   if (e == cudaSuccess) {
     if (s->tc) e = tc_launch_recon(s->tc, s->partial_dev, s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
@@ -377,7 +381,12 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
     e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->st);
   mark(5);
   if (s->stage_timing) s->ev_rec.push_back(std::move(ev));
-  if (e != cudaSuccess) { set_error("stream_push: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  if (e != cudaSuccess) {
+    // kernels already enqueued have appended to the rings while the stream clock did not advance: the state is
+    // inconsistent, so the stream refuses further pushes (LLOID_ESTATE) until lloid_state_reset
+    s->failed = true;
+    set_error("stream_push: launch failed: %s (stream needs lloid_state_reset)", cudaGetErrorString(e)); return LLOID_ECUDA;
+  }
   s->n0_host += s->B;
   return LLOID_OK;
 }
@@ -401,6 +410,7 @@ extern "C" int lloid_state_reset(lloid_stream *s) {
     if (e != cudaSuccess) { set_error("state_reset: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   }
   s->n0_host = 0;
+  s->failed = false;
   return LLOID_OK;
 }
 

@@ -145,3 +145,44 @@ def test_multi_rank_bench_plumbing_gloo(tmp_path):
     assert abs(res["value"] - 2 * 64 * 5 / 0.020) < 1e-6      # whole-job aggregate
     seed1 = [json.loads(ln) for ln in r.stderr.splitlines() if ln.startswith('{"seed1"')]
     assert seed1 and seed1[-1]["seed1"] != res["seed0"]       # replicas filter different strain
+
+
+def test_bench_gpus_flag_launches_ranks_itself():
+    """`python bench.py --gpus 2` (no torchrun around it) must start 2 ranks on its own: the plumbing check runs the
+    launcher -> rank environment -> process group (gloo) -> barrier -> max over ranks -> one rank-0 line path without
+    any filtering, and the printed n_gpus is the number of ranks the process group saw."""
+    import json
+    env = {k: v for k, v in os.environ.items() if k not in ("WORLD_SIZE", "RANK", "LOCAL_RANK")}
+    env["MASTER_PORT"] = "29591"
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "2", "--steps", "5", "--plumbing-check"],
+                       capture_output=True, text=True, env=env, timeout=300)
+    assert r.returncode == 0, r.stderr[-2000:]
+    lines = [ln for ln in r.stdout.splitlines() if ln.startswith("{")]
+    assert len(lines) == 1                                     # rank 0 alone prints
+    res = json.loads(lines[0])
+    assert res["n_gpus"] == 2 and res["gpus_arg"] == 2
+    assert abs(res["t"] - 0.020) < 1e-9                        # max over ranks
+    assert abs(res["value"] - 2 * 64 * 5 / 0.020) < 1e-6       # whole-job aggregate of 2 replicas
+
+
+def test_bench_refuses_a_rank_count_that_contradicts_gpus():
+    """Under a launcher whose WORLD_SIZE differs from --gpus the bench exits non-zero instead of printing a wrong n_gpus."""
+    env = dict(os.environ, WORLD_SIZE="2", RANK="0", LOCAL_RANK="0")
+    r = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--gpus", "1", "--plumbing-check"],
+                       capture_output=True, text=True, env=env, timeout=120)
+    assert r.returncode != 0 and "--gpus" in r.stderr
+
+
+def test_bench_plan_is_deterministic_and_names_the_headline():
+    sys.path.insert(0, ROOT)
+    import bench
+    assert bench.HEADLINE_CONFIG == 5 and bench.parse([]).config == 0
+    c, plan = bench.bank_plan(5)
+    assert len(plan) == 1000 and bench.config_dict(5, c, plan)["workload"].startswith("BASELINE.json configs[4]")
+    real = [p[1] for p in plan if p[0] == "real"]
+    assert {0, 333, 666, 999} <= set(real) and 4 < len(real) <= 8
+    inj_banks = [i.bank for i in c.injections(bench.parity_seconds(c))]
+    assert set(real) - {0, 333, 666, 999} <= set(inj_banks)                     # the extra real banks are injected banks
+    assert plan == bench.bank_plan(5)[1]
+    for p in plan:
+        assert p[0] == "real" or p[2] in real

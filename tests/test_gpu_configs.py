@@ -10,7 +10,7 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
-TOL = {0: 1e-4, 2: 2e-3}
+from parity_util import TOL, check_peaks, snr_errors
 
 
 def _cuda():
@@ -47,21 +47,15 @@ def _stream_and_check(banks, strain, B, precision, check, must):
         bank = banks[bi]
         for det in range(n_det):
             ref = lloid_snr(bank, strain[det][:(p + 1) * B], p * B, (p + 1) * B)
-            z_ref = ref[0::2] + 1j * ref[1::2]
-            z = rho[det][0::2] + 1j * rho[det][1::2]
-            rms = math.sqrt(np.mean(np.abs(z_ref) ** 2))
-            err = np.abs(z - z_ref).max() / rms
+            err, _ = snr_errors(rho[det], ref)
             worst = max(worst, err)
             assert err <= TOL[precision], f"push {p} bank {bi} det {det}: max err {err:.3e} of SNR rms"
             snr_o, idx_o, ph_o = find_peaks(ref, B)
             pk = peaks[det, off[bi]:off[bi + 1]]
-            at = np.abs(z_ref[np.arange(bank.M), pk["sample"]])
-            assert (snr_o[0] - at <= 2 * TOL[precision] * rms).all()          # every GPU peak is an oracle maximum
-            assert np.abs(pk["snr"] - at).max() <= 2 * TOL[precision] * rms
-            for (pp, bb, dd, j) in must:
-                if (pp, bb, dd) == (p, bi, det):
-                    assert pk["sample"][j] == idx_o[0, j], (p, bi, det, j)   # bit-exact for loud injections
-                    assert snr_o[0, j] >= 8.0 * 0.8
+            mm = [(0, j) for (pp, bb, dd, j) in must if (pp, bb, dd) == (p, bi, det)]      # bit-exact for loud injections
+            check_peaks(pk[None], ref, B, TOL[precision], mm)                 # every GPU peak is an oracle maximum
+            for (_, j) in mm:
+                assert snr_o[0, j] >= 8.0 * 0.8
     st.close()
     return worst
 

@@ -10,9 +10,10 @@ import pytest
 
 pytestmark = pytest.mark.gpu
 
+from parity_util import TOL, check_peaks, snr_errors
+
 # precision 1 (operands rounded once to fp16) is NOT a north-star mode: its error near loud injections exceeds 2e-3
 # (DESIGN.md section 4); it is gated at 1e-2 only to prove the kernels' single-plane path.
-TOL = {0: 1e-4, 1: 1e-2, 2: 2e-3}
 
 
 def _torch_cuda():
@@ -22,10 +23,10 @@ def _torch_cuda():
     return torch
 
 
-def run_gpu(banks, strain, B, precision, want_bank=0, n_push=None):
+def run_gpu(banks, strain, B, precision, want_bank=0, n_push=None, **kw):
     """Push strain [n_det][n] in buffers of B; return (rho [n_det][2M][n_push*B], peaks [n_push][n_det][Mtot])."""
     import paper_2511_04730_b200 as lib
-    st = lib.LloidStream(banks, strain.shape[0], B, precision=precision)
+    st = lib.LloidStream(banks, strain.shape[0], B, precision=precision, **kw)
     n_push = strain.shape[1] // B if n_push is None else n_push
     rho, peaks = [], []
     for p in range(n_push):
@@ -36,31 +37,8 @@ def run_gpu(banks, strain, B, precision, want_bank=0, n_push=None):
     return np.concatenate(rho, axis=2), np.stack(peaks)
 
 
-def check_snr(rho_gpu, rho_ref, tol):
-    z_ref = rho_ref[0::2] + 1j * rho_ref[1::2]
-    z_gpu = rho_gpu[0::2] + 1j * rho_gpu[1::2]
-    rms = np.sqrt(np.mean(np.abs(z_ref) ** 2))
-    err = np.abs(z_gpu - z_ref)
-    return err.max() / rms, np.sqrt(np.mean(err ** 2)) / rms
-
-
-def check_peaks(pk, rho_ref, B, tol_abs, must_match=()):
-    """pk: [n_push][M] structured GPU peaks of one bank+detector; rho_ref [2M][n_push*B] float64."""
-    from oracle import find_peaks
-    snr, idx, ph = find_peaks(rho_ref, B)
-    n_push, M = snr.shape
-    for (p, j) in must_match:
-        assert pk["sample"][p, j] == idx[p, j], (p, j, pk["sample"][p, j], idx[p, j])
-    z = rho_ref[0::2] + 1j * rho_ref[1::2]
-    for p in range(n_push):
-        k = pk["sample"][p].astype(np.int64)
-        assert (k >= 0).all() and (k < B).all()
-        at = np.abs(z[np.arange(M), p * B + k])
-        assert (snr[p] - at <= tol_abs).all(), f"push {p}: GPU peak sample is not a maximum of the oracle SNR"
-        assert np.abs(pk["snr"][p] - at).max() <= tol_abs
-        dphi = np.angle(np.exp(1j * (pk["phase"][p] - np.angle(z[np.arange(M), p * B + k]))))
-        assert np.abs(dphi * at).max() <= 2 * tol_abs
-    return float(np.mean(pk["sample"] == idx))
+def check_snr(rho_gpu, rho_ref, tol=None):
+    return snr_errors(rho_gpu, rho_ref)
 
 
 @pytest.mark.parametrize("precision", [0, 2, 1])
@@ -76,9 +54,8 @@ def test_config1_full_snr_and_peaks(cfg1, precision):
     emax, erms = check_snr(rho_gpu[0], rho_ref, TOL[precision])
     print(f"config1 precision={precision}: max err {emax:.3e} rms err {erms:.3e} (of SNR rms)")
     assert emax <= TOL[precision]
-    rms = np.sqrt(np.mean(rho_ref[0::2] ** 2 + rho_ref[1::2] ** 2))
     must = [(inj.k0 // B, inj.template) for inj in cfg1["inj"]]
-    frac = check_peaks(peaks[:, 0, :], rho_ref, B, TOL[precision] * rms * 2, must)
+    frac = check_peaks(peaks[:, 0, :], rho_ref, B, TOL[precision], must)
     print(f"  peak sample agreement {frac:.4f}")
     for inj in cfg1["inj"]:
         p, j = inj.k0 // B, inj.template
@@ -126,7 +103,7 @@ def test_multirate_bank_two_detectors(precision):
         emax, erms = check_snr(rho_gpu[det], rho_ref, TOL[precision])
         print(f"multirate det {det}: max err {emax:.3e} rms {erms:.3e}")
         assert emax <= TOL[precision]
-        check_peaks(peaks[:, det, :], rho_ref, B, TOL[precision] * 2 * np.sqrt(2.0))
+        check_peaks(peaks[:, det, :], rho_ref, B, TOL[precision])
 
 
 def test_ragged_buffer_threshold_and_host_push():
@@ -157,7 +134,7 @@ def test_ragged_buffer_threshold_and_host_push():
             ref = lloid_snr(bank, strain[det])
             emax, _ = check_snr(rho_gpu[det], ref, TOL[precision])
             assert emax <= TOL[precision]
-            check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0) * 3)
+            check_peaks(peaks[:, det, :], ref, B, TOL[precision])
         assert (peaks["snr"][4, 0] >= thr).any()
 
 
@@ -225,7 +202,7 @@ def test_large_decimation_and_single_big_upsample_stage(precision):
         emax, erms = check_snr(rho_gpu[det], ref, TOL[precision])
         print(f"D=128 bank det {det} precision {precision}: max err {emax:.3e}")
         assert emax <= TOL[precision]
-        check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0))
+        check_peaks(peaks[:, det, :], ref, B, TOL[precision])
 
 
 def test_n_down_option():
@@ -263,4 +240,66 @@ def test_degenerate_sizes(precision):
         ref = lloid_snr(bank, strain[det])
         emax, _ = check_snr(rho_gpu[det], ref, TOL[precision])
         assert emax <= TOL[precision]
-        check_peaks(peaks[:, det, :], ref, B, TOL[precision] * 2 * np.sqrt(2.0))
+        check_peaks(peaks[:, det, :], ref, B, TOL[precision])
+
+
+def test_threshold_mismatch_is_rejected():
+    """All banks of a stream share one trigger threshold (include/lloid.h): mixing thresholds is LLOID_EINVAL."""
+    _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from workloads import random_bank
+    bank = random_bank(5, 9, [(2048, 128, 4)]).as_f32()
+    h1 = lib.lloid_bank_create(bank.f0, bank.M, lib.bank_slices(bank), lib.LLOID_PREC_F16_SPLIT, threshold=0.0)
+    h2 = lib.lloid_bank_create(bank.f0, bank.M, lib.bank_slices(bank), lib.LLOID_PREC_F16_SPLIT, threshold=4.0)
+    with pytest.raises(lib.LloidError) as e:
+        lib.lloid_stream_create([h1, h2], 1, 256)
+    assert e.value.code == lib.LLOID_EINVAL and "threshold" in str(e.value)
+    lib.lloid_bank_destroy(h1); lib.lloid_bank_destroy(h2)
+
+
+_TIGHT_STRAIN = r"""
+import ctypes, sys
+import numpy as np, torch
+sys.path.insert(0, {root!r})
+import paper_2511_04730_b200 as lib
+from workloads import make_strain, random_bank
+torch.cuda.init(); torch.zeros(1, device="cuda")
+rt = ctypes.CDLL("libcudart.so.12")
+rt.cudaMalloc.argtypes = [ctypes.POINTER(ctypes.c_void_p), ctypes.c_size_t]
+rt.cudaMemcpy.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int]
+B, n_det, n_push = 128, 3, 40
+bank = random_bank(77, 12, [(2048, 4096, 6), (1024, 2048, 5), (64, 64, 4), (32, 64, 3)]).as_f32()    # B/D = 2 and 4
+strain = np.stack([make_strain(770 + d, B * n_push) for d in range(n_det)])
+st = lib.LloidStream([bank], n_det, B)
+ref = np.stack([st.push(strain[:, p * B:(p + 1) * B]).copy() for p in range(n_push)])
+st.reset()
+nbytes = n_det * B * 4
+size = 2 << 20                                        # one 2 MiB allocation granule; the strain sits in its last bytes
+base = ctypes.c_void_p()
+assert rt.cudaMalloc(ctypes.byref(base), size) == 0
+ptr = base.value + size - nbytes
+pk = torch.zeros((n_det, st.Mtot, st.peaks_dev.shape[-1]), dtype=torch.int32, device="cuda")
+for p in range(n_push):
+    buf = np.ascontiguousarray(strain[:, p * B:(p + 1) * B])
+    assert rt.cudaMemcpy(ptr, buf.ctypes.data, nbytes, 1) == 0
+    lib.lloid_stream_push(st.handle, ptr, pk.data_ptr())
+    torch.cuda.synchronize()                          # an over-read of an unmapped page faults here
+    got = pk.cpu().numpy().view(lib.PEAK_DTYPE).reshape(n_det, st.Mtot)
+    assert np.array_equal(got["sample"], ref[p]["sample"]) and np.array_equal(got["snr"], ref[p]["snr"])
+print("TIGHT_OK")
+"""
+
+
+def test_decimator_does_not_read_past_an_exact_size_strain_buffer(tmp_path):
+    """with B/D in {2, 4} a decimator CTA stages 8 outputs, 6 / 4 of which do not exist; their strain lies
+    beyond [n_det][B].  The strain is placed in the LAST bytes of an exact-size cudaMalloc (own process: a fault would
+    poison the CUDA context) and the peaks must equal those of an ordinary torch-allocated push."""
+    _torch_cuda()
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    script = tmp_path / "tight.py"
+    script.write_text(_TIGHT_STRAIN.format(root=root))
+    r = subprocess.run([sys.executable, str(script)], capture_output=True, text=True, timeout=600)
+    assert r.returncode == 0 and "TIGHT_OK" in r.stdout, (r.stdout[-1500:], r.stderr[-3000:])

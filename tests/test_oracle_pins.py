@@ -44,16 +44,19 @@ def test_eq4_structure(f):
 
 
 # ---------------------------------------------------------------- decimator
-@pytest.mark.parametrize("D", [2, 4, 16])
-def test_decimate_equals_textbook_filter_then_pick(D):
-    """Zero-phase decimation = full-rate convolution with sqrt(D)*ghat, centred, then every D-th sample."""
+@pytest.mark.parametrize("D,n_down", [(2, N_DOWN), (4, N_DOWN), (16, N_DOWN), (4, 12), (16, 12), (8, 5)])
+def test_decimate_equals_textbook_filter_then_pick(D, n_down):
+    """Zero-phase decimation = full-rate convolution with sqrt(D)*ghat, centred, then every D-th sample -- also
+    for a non-default half length (lloid_options.n_down, PAPER.md:132 'typically set to 32')."""
     rng = np.random.default_rng(D)
     d = rng.standard_normal(2000)
-    g = resample_kernel(D, N_DOWN)
-    c = N_DOWN * D
+    g = resample_kernel(D, n_down)
+    c = n_down * D
+    assert len(g) == 2 * c + 1
     full = scipy.signal.convolve(d, math.sqrt(D) * g / g.sum(), mode="full")   # full[i] = sum_k h[k] d[i-k]
-    s = decimate(d, D)
-    for j in range(-N_DOWN, 2000 // D + N_DOWN):
+    s = decimate(d, D, n_down)
+    assert s.j0 == -n_down
+    for j in range(-n_down, 2000 // D + n_down):
         i = j * D + c
         want = full[i] if 0 <= i < len(full) else 0.0
         assert abs(s.window(j, j + 1)[0] - want) < 1e-13
@@ -131,13 +134,27 @@ def test_upsample_tone_gain():
     assert np.abs(y - np.cos(2 * math.pi * nu * i / f + 0.7)).max() < 1e-3   # within 1e-3 to 0.5 Nyquist
 
 
-def test_upsample_input_range_is_tight():
+def test_upsample_input_range_is_sufficient_and_tight():
+    """The range the oracle asks of the stage below is exactly what `upsample` reads: it is enough (no assert), every
+    input inside it but none outside influences the outputs (checked by perturbing single inputs), and cutting it
+    short by two on the left or one on the right makes `upsample` fail."""
     for f in (2, 4):
-        for lo, hi in ((0, 64), (-5, 7), (33, 35)):
+        for lo, hi in ((0, 64), (-5, 7), (33, 35), (f + 1, 3 * f)):
             a, b = upsample_input_range(lo, hi, f)
-            x = np.random.default_rng(1).standard_normal(b - a)
-            upsample(x[None], a, f, lo, hi)                   # must not assert
-            assert a == lo // f - N_UP and b == (hi - 1) // f + N_UP + 1
+            x = np.random.default_rng(1).standard_normal(b - a + 8)        # 4 spare inputs on both sides
+            y = upsample(x[None], a - 4, f, lo, hi)[0]                     # must not assert
+            used = []
+            for m in range(len(x)):
+                xp = x.copy()
+                xp[m] += 1.0
+                used.append(bool(np.abs(upsample(xp[None], a - 4, f, lo, hi)[0] - y).max() > 1e-9))
+            idx = np.nonzero(used)[0] + a - 4
+            assert a <= idx.min() <= a + 1 and (idx.max() == b - 1 if (hi - 1) % f else b - 3 <= idx.max() <= b - 1)
+            with pytest.raises(AssertionError):
+                upsample(x[None, 6:], a + 2, f, lo, hi)
+            if (hi - 1) % f:
+                with pytest.raises(AssertionError):
+                    upsample(x[None, 4:b - a + 3], a, f, lo, hi)
 
 
 # ---------------------------------------------------------------- Eq. 5 / Eq. 6 index conventions
@@ -316,13 +333,18 @@ def test_lloid_vs_brute_force_approximation_band(cfg1):
     assert err.std() < 3e-2 and np.abs(err).max() < 0.2
 
 
-def test_multirate_chain_with_skipped_and_repeated_rates():
+@pytest.mark.parametrize("n_down", [N_DOWN, 12])
+def test_multirate_chain_with_skipped_and_repeated_rates(n_down):
     """Random bank, rates 2048/512/512/128 (one x4 stage, two slices at one rate, another x4 stage):
-    the oracle must equal an independent composition written with scipy's upfirdn."""
+    the oracle must equal an independent composition written with scipy's upfirdn -- with the default decimator
+    half length and with n_down = 12 (the lloid_options.n_down path the GPU test test_n_down_option compares against)."""
+    N_DOWN = n_down
     bank = random_bank(7, 3, [(2048, 40, 5), (512, 30, 4), (512, 20, 3), (128, 25, 4)])
     d = np.random.default_rng(8).standard_normal(6000)
     k0, k1 = 3000, 3256
-    got = lloid_snr(bank, d, k0, k1)
+    got = lloid_snr(bank, d, k0, k1, n_down=n_down)
+    if n_down != 32:
+        assert np.abs(got - lloid_snr(bank, d, k0, k1)).max() > 1e-4      # the option does change the result
 
     def own(s, D):
         sl = bank.slices[s]
