@@ -118,10 +118,12 @@ def _fullsize(cfg_no, n_rows=6, tail_pushes=1):
                 pk = np.stack([pk_all[i, det] for i in sl])                         # [per_s][M]
                 agree.append(check_peaks(pk, ref, B, TOL[2], must))
                 snr_o, idx_o, _ = find_peaks(ref, B)
-                for (p, j) in must:                                                 # and the injection is actually found
-                    i = next(x for x in inj_here if x.template == j)
-                    # (heavy, narrow-band templates peak a few samples off the injected one in N(0,1) noise)
-                    assert abs(int(idx_o[p, j]) - i.k0 % B) <= 8 and snr_o[p, j] > 0.75 * i.amp - 2.0, (bi, det, j, i.amp, snr_o[p, j])
+                for i in inj_here:                                                  # and the oracle does see the injection:
+                    # loud within a few ms of the injected sample (heavy, narrow-band templates peak several samples off
+                    # it in N(0,1) noise, possibly in the neighbouring buffer -- the bit-exact check above is GPU vs oracle)
+                    a, b = max(i.k0 % f0 - 16, 0), min(i.k0 % f0 + 17, f0)
+                    z = ref[2 * i.template, a:b] + 1j * ref[2 * i.template + 1, a:b]
+                    assert np.abs(z).max() > 0.75 * i.amp - 2.0, (bi, det, i.template, i.amp, float(np.abs(z).max()))
                 n_checked += 1
     st.close()
     kinds = {b: ("standin" if b in standins else ("injected" if any(i.bank == b for i in injs) else "real")) for b in check_banks}
