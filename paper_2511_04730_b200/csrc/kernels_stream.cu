@@ -403,6 +403,16 @@ __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_d
   peaks[t] = o;
 }
 
+__global__ void fill_partial_kernel(PeakPartial *partial, size_t n) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) { PeakPartial e; e.p = -3.f; e.idx = 0x7fffffff; e.re = 0.f; e.im = 0.f; partial[i] = e; }
+}
+cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st) {
+  if (n == 0) return cudaSuccess;
+  fill_partial_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partial, n);
+  return cudaGetLastError();
+}
+
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
                             lloid_peak *peaks, long long *n0, int B, cudaStream_t st) {
   int g = 1;

@@ -9,6 +9,7 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cstdlib>
 #include <cstring>
 #include <queue>
 #include <type_traits>
@@ -29,9 +30,11 @@ struct TcReconTile { int bank, det, m0, t0, nt, slot; };   // nt consecutive tim
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
   CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 64 x 128
   CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 64 x 128
+  CUtensorMap mapY64;                        // same array, box 64 x 64 (resident-R kernel: 64-sample tiles)
+  const __half *R16;                         // [planes][2][Mpad][Kpad]
   int M, Mpad, Kpad, tmpl_off;
   float inv_scale;
-  int pad_[11];
+  int pad_[9];
 };
 struct TcCorrClass {
   CUtensorMap mapU;                          // [planes*Lpad rows][Npad] fp16, box 64 x 128
@@ -47,7 +50,7 @@ template <int PLANES>
 __global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                 int n_det, int B,
-                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank) {
+                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank, int terms) {
   constexpr int STAGES = PLANES == 2 ? 2 : 4;
   constexpr int STAGE_BYTES = 3 * PLANES * TILE_BYTES;        // Rre, Rim, Y per plane
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -121,10 +124,8 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
             if (PLANES == 2) {
               const uint64_t re_lo = db + ((3 * TILE_BYTES + k * 32) >> 4), im_lo = db + ((4 * TILE_BYTES + k * 32) >> 4),
                              y_lo = db + ((5 * TILE_BYTES + k * 32) >> 4);
-              mma_f16_ss(d_re, re_hi, y_lo, idesc, true);
-              mma_f16_ss(d_im, im_hi, y_lo, idesc, true);
-              mma_f16_ss(d_re, re_lo, y_hi, idesc, true);
-              mma_f16_ss(d_im, im_lo, y_hi, idesc, true);
+              if (terms & 0x20) { mma_f16_ss(d_re, re_hi, y_lo, idesc, true); mma_f16_ss(d_im, im_hi, y_lo, idesc, true); }
+              if (terms & 0x40) { mma_f16_ss(d_re, re_lo, y_hi, idesc, true); mma_f16_ss(d_im, im_lo, y_hi, idesc, true); }
             }
           }
           mma_commit(&empty[stage]);
@@ -201,6 +202,235 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 }
 
 // ------------------------------------------------------------------------------------------------
+// a3 + a5, resident-R variant (banks with Kpad <= TS_KMAX, hi + lo planes).  A work item is one (bank, 128-template tile)
+// and a run of (detector, time tile) pairs; the template tile's reconstruction rows stay ON CHIP for the whole item:
+//   R_hi (re, im) in TENSOR MEMORY as the A operand of tcgen05.mma (columns 256.., written once per item by the epilogue
+//        warps with tcgen05.st) -- 4 of the 6 MMAs of a K step then read only the Y tile from shared memory;
+//   R_lo (re, im) resident in shared memory (TMA, once per item) for the two R_lo x Y_hi MMAs.
+// Only the upsampled-Y tiles [64 samples][64 K] (hi, lo) stream through the TMA ring.  Tile = 128 templates x 64 samples,
+// re / im accumulators double buffered in TMEM columns 0..255.
+// Peak search: per 16-sample chunk the epilogue thread computes |z|^2 (packed fp32x2), the chunk maximum (3-input max),
+// and only when it beats the running maximum saves the chunk's (re, im) to a per-thread shared-memory slot; the first
+// sample attaining the maximum is located once per run from the saved chunk (same arithmetic, bit-identical p).
+// ------------------------------------------------------------------------------------------------
+static constexpr int TS_NT = 64;                        // samples per tile
+static constexpr int TS_KMAX = 256;                     // R_hi (re + im) fills TMEM columns 256..511
+static constexpr int TS_THREADS = 320;                  // warps: 0 TMA, 1 MMA, 2-9 epilogue / R loaders
+static constexpr int TS_YTILE = TS_NT * BK * 2;         // one plane of a Y stage: 8 KB
+static constexpr int TS_YSTAGE = 2 * TS_YTILE;          // hi + lo
+static constexpr int TS_CHUNK = 16;                     // samples per peak-search chunk
+static constexpr int TS_REC_BYTES = 256 * TS_CHUNK * 8; // saved record chunk per epilogue thread: 32 KB
+static constexpr int TS_MAX_YSTAGES = 8;
+
+struct TsItem { int bank, m0, det0, ndet, t0, nt, slot; };   // nt tiles of 64 samples from sample t0, for detectors det0..det0+ndet-1
+
+__global__ void __launch_bounds__(TS_THREADS, 1)
+recon_ts_kernel(const TcReconBank *__restrict__ banks, const TsItem *__restrict__ items, const int *__restrict__ cta_begin,
+                int n_det, int B, PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug,
+                int debug_bank, int rlo_bytes, int n_ys) {
+  extern __shared__ __align__(1024) uint8_t smem_raw[];
+  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t *rlo = smem;                                           // [2 parts][nkb][128 rows x 64 K] fp16, 128-B swizzle
+  uint8_t *ybuf = smem + rlo_bytes;                              // [n_ys][hi, lo][64 samples x 64 K]
+  float4 *rec = (float4 *)(ybuf + n_ys * TS_YSTAGE);             // [8][256 threads] {re0, im0, re1, im1}
+  uint64_t *bars = (uint64_t *)((uint8_t *)rec + TS_REC_BYTES);
+  uint64_t *yfull = bars, *yempty = bars + TS_MAX_YSTAGES, *tfull = bars + 2 * TS_MAX_YSTAGES, *tempty = tfull + 2,
+           *rfull = tempty + 2, *rlofull = rfull + 1, *rdone = rlofull + 1;
+  uint32_t *tmem_slot = (uint32_t *)(rdone + 1);
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+
+  if (warp == 0 && lane == 0) {
+    for (int i = 0; i < n_ys; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 1); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 8); }
+    mbar_init(rfull, 8); mbar_init(rlofull, 1); mbar_init(rdone, 1);
+    mbar_fence_init();
+  }
+  if (warp == 1) tmem_alloc(tmem_slot, 512);
+  tc_fence_before_sync();
+  __syncthreads();
+  tc_fence_after_sync();
+  const uint32_t tmem = *tmem_slot;
+  const int i_begin = cta_begin[blockIdx.x], i_end = cta_begin[blockIdx.x + 1];
+
+  if (warp == 0) {
+    // ===== TMA producer: R_lo once per item, then the Y tiles of every (detector, time tile)
+    if (lane == 0) {
+      int stage = 0; uint32_t phase = 0;
+      for (int ii = i_begin; ii < i_end; ++ii) {
+        const TsItem it = items[ii];
+        const TcReconBank *bk = &banks[it.bank];
+        const int nkb = (bk->Kpad + BK - 1) / BK;
+        if (ii > i_begin) mbar_wait(rdone, (uint32_t)(ii - i_begin - 1) & 1);     // previous item's MMAs have read R_lo
+        mbar_arrive_expect_tx(rlofull, 2 * nkb * TILE_BYTES);
+        for (int part = 0; part < 2; ++part)
+          for (int kb = 0; kb < nkb; ++kb)
+            tma_load_2d(rlo + (part * nkb + kb) * TILE_BYTES, &bk->mapR, rlofull, kb * BK, (2 + part) * bk->Mpad + it.m0);
+        for (int d = 0; d < it.ndet; ++d)
+          for (int tt = 0; tt < it.nt; ++tt) {
+            const int row = (it.det0 + d) * B + it.t0 + tt * TS_NT;
+            for (int kb = 0; kb < nkb; ++kb) {
+              mbar_wait(&yempty[stage], phase ^ 1);
+              mbar_arrive_expect_tx(&yfull[stage], TS_YSTAGE);
+              uint8_t *sdst = ybuf + stage * TS_YSTAGE;
+              tma_load_2d(sdst, &bk->mapY64, &yfull[stage], kb * BK, row);
+              tma_load_2d(sdst + TS_YTILE, &bk->mapY64, &yfull[stage], kb * BK, n_det * B + row);
+              if (++stage == n_ys) { stage = 0; phase ^= 1; }
+            }
+          }
+      }
+    }
+  } else if (warp == 1) {
+    // ===== MMA issuer
+    if (lane == 0) {
+      constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TS_NT);
+      int stage = 0; uint32_t phase = 0; int t_it = 0;
+      for (int ii = i_begin; ii < i_end; ++ii) {
+        const TsItem it = items[ii];
+        const int Kpad = banks[it.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
+        const uint32_t ip = (uint32_t)(ii - i_begin) & 1;
+        mbar_wait(rfull, ip);
+        mbar_wait(rlofull, ip);
+        tc_fence_after_sync();
+        const uint32_t a_re0 = tmem + 256, a_im0 = a_re0 + (Kpad >> 1);
+        const uint64_t rl_re0 = desc_kmajor_sw128(smem_u32(rlo)), rl_im0 = desc_kmajor_sw128(smem_u32(rlo + nkb * TILE_BYTES));
+        const int ntile = it.ndet * it.nt;
+        for (int tl = 0; tl < ntile; ++tl, ++t_it) {
+          const int buf = t_it & 1;
+          mbar_wait(&tempty[buf], ((t_it >> 1) & 1) ^ 1);
+          tc_fence_after_sync();
+          const uint32_t d_re = tmem + buf * 128, d_im = d_re + 64;
+          for (int kb = 0; kb < nkb; ++kb) {
+            mbar_wait(&yfull[stage], phase);
+            tc_fence_after_sync();
+            const uint64_t yd = desc_kmajor_sw128(smem_u32(ybuf + stage * TS_YSTAGE));
+            const int nk = min(BK / 16, (Kpad - kb * BK) / 16);
+#pragma unroll
+            for (int k = 0; k < BK / 16; ++k) {
+              if (k >= nk) break;
+              const bool acc = (kb | k) != 0;
+              const uint32_t ks = (uint32_t)(kb * (BK / 16) + k) * 8;            // 16 fp16 of K = 8 TMEM columns
+              const uint64_t y_hi = yd + 2 * k, y_lo = y_hi + (TS_YTILE >> 4);
+              const uint64_t off = (uint64_t)((kb * TILE_BYTES + k * 32) >> 4);
+              mma_f16_ts(d_re, a_re0 + ks, y_hi, idesc, acc);
+              mma_f16_ts(d_im, a_im0 + ks, y_hi, idesc, acc);
+              mma_f16_ts(d_re, a_re0 + ks, y_lo, idesc, true);
+              mma_f16_ts(d_im, a_im0 + ks, y_lo, idesc, true);
+              mma_f16_ss(d_re, rl_re0 + off, y_hi, idesc, true);
+              mma_f16_ss(d_im, rl_im0 + off, y_hi, idesc, true);
+            }
+            mma_commit(&yempty[stage]);
+            if (++stage == n_ys) { stage = 0; phase ^= 1; }
+          }
+          mma_commit(&tfull[buf]);
+        }
+        mma_commit(rdone);
+      }
+    }
+  } else {
+    // ===== epilogue warps (8): thread = template (TMEM lane) x one half (32 samples) of the tile; they also place R_hi of
+    // each item in tensor memory (warps 2-5: real rows, 6-9: imaginary rows)
+    const int q = warp & 3, half = (warp - 2) >> 2, etid = threadIdx.x - 64;
+    const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+    int t_it = 0;
+    for (int ii = i_begin; ii < i_end; ++ii) {
+      const TsItem it = items[ii];
+      const TcReconBank *bk = &banks[it.bank];
+      const int M = bk->M, Kpad = bk->Kpad, tmpl_off = bk->tmpl_off;
+      const int m = it.m0 + q * 32 + lane;
+      const float sc = bk->inv_scale;
+      {
+        // every MMA of the previous item has completed (this warp waited for tfull of its last tile): R_hi may be replaced
+        const uint4 *src = reinterpret_cast<const uint4 *>(bk->R16 + ((size_t)half * bk->Mpad + m) * Kpad);
+        const uint32_t tdst = tmem + lane_base + 256 + half * (Kpad >> 1);
+        const int n16 = Kpad >> 4;
+#pragma unroll 4
+        for (int c = 0; c < n16; ++c) {
+          const uint4 a = __ldg(src + 2 * c), b = __ldg(src + 2 * c + 1);
+          const uint32_t v[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
+          tmem_st_32x8(tdst + c * 8, v);
+        }
+        tmem_st_wait();
+        tc_fence_before_sync();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(rfull);
+      }
+      const bool dbg = snr_debug != nullptr && it.bank == debug_bank && m < M;
+      for (int d = 0; d < it.ndet; ++d) {
+        const int det = it.det0 + d;
+        float bp = -1.f;
+        int bt0 = 0;
+        for (int tt = 0; tt < it.nt; ++tt, ++t_it) {
+          const int buf = t_it & 1;
+          const int tbase = it.t0 + tt * TS_NT + half * 32;
+          mbar_wait(&tfull[buf], (t_it >> 1) & 1);
+          tc_fence_after_sync();
+          const uint32_t t_re = tmem + lane_base + buf * 128 + half * 32;
+          uint32_t vr[32], vi[32];
+          tmem_ld_32x32(t_re, vr);
+          tmem_ld_32x32(t_re + 64, vi);
+          tmem_ld_wait();
+          tc_fence_before_sync();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty[buf]);                 // the accumulators are in registers: release the buffer
+#pragma unroll
+          for (int c = 0; c < 32 / TS_CHUNK; ++c) {
+            const int t0c = tbase + c * TS_CHUNK;
+            float p[TS_CHUNK];
+#pragma unroll
+            for (int i = 0; i < TS_CHUNK; i += 2)
+              abs2_x2(__uint_as_float(vr[c * TS_CHUNK + i]), __uint_as_float(vr[c * TS_CHUNK + i + 1]),
+                      __uint_as_float(vi[c * TS_CHUNK + i]), __uint_as_float(vi[c * TS_CHUNK + i + 1]), p[i], p[i + 1]);
+            if (t0c + TS_CHUNK > B) {
+#pragma unroll
+              for (int i = 0; i < TS_CHUNK; ++i) if (t0c + i >= B) p[i] = -1.f;
+            }
+            float cm = p[0];
+#pragma unroll
+            for (int i = 1; i + 1 < TS_CHUNK; i += 2) cm = fmaxf(cm, fmaxf(p[i], p[i + 1]));
+            cm = fmaxf(cm, p[TS_CHUNK - 1]);
+            const bool rec_now = cm > bp;                          // strict: an earlier chunk keeps a tie (first maximum)
+            if (__any_sync(0xffffffffu, rec_now)) {
+              if (rec_now) {
+                bp = cm; bt0 = t0c;
+#pragma unroll
+                for (int j = 0; j < TS_CHUNK / 2; ++j)
+                  rec[j * 256 + etid] = make_float4(__uint_as_float(vr[c * TS_CHUNK + 2 * j]), __uint_as_float(vi[c * TS_CHUNK + 2 * j]),
+                                                    __uint_as_float(vr[c * TS_CHUNK + 2 * j + 1]), __uint_as_float(vi[c * TS_CHUNK + 2 * j + 1]));
+              }
+            }
+          }
+          if (dbg) {
+            float *o = snr_debug + ((size_t)det * 2 * M + 2 * m) * B;
+#pragma unroll
+            for (int i = 0; i < 32; ++i)
+              if (tbase + i < B) { o[tbase + i] = __uint_as_float(vr[i]) * sc; o[B + tbase + i] = __uint_as_float(vi[i]) * sc; }
+          }
+        }
+        if (m < M) {
+          PeakPartial best;
+          best.p = -1.f; best.idx = 0; best.re = 0.f; best.im = 0.f;
+          if (bp >= 0.f) {
+            bool found = false;
+#pragma unroll
+            for (int j = 0; j < TS_CHUNK / 2; ++j) {
+              const float4 v = rec[j * 256 + etid];
+              const float p0 = __fmaf_rn(v.y, v.y, __fmul_rn(v.x, v.x)), p1 = __fmaf_rn(v.w, v.w, __fmul_rn(v.z, v.z));
+              if (!found && p0 == bp) { found = true; best.idx = bt0 + 2 * j; best.re = v.x * sc; best.im = v.y * sc; }
+              if (!found && p1 == bp) { found = true; best.idx = bt0 + 2 * j + 1; best.re = v.z * sc; best.im = v.w * sc; }
+            }
+            best.p = best.re * best.re + best.im * best.im;
+          }
+          partial[((size_t)det * Mtot + tmpl_off + m) * n_tt + it.slot * 2 + half] = best;
+        }
+      }
+    }
+  }
+  tc_fence_before_sync();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem, 512);
+}
+
+// ------------------------------------------------------------------------------------------------
 // a2.  Persistent CTAs (one per SM) over work UNITS = (class, 128 stacked basis rows, tap segment of <= 1024 taps,
 // up to 4 sub-tiles), a sub-tile being 128 (or fewer) output columns of one detector.  All sub-tiles of a unit share
 // the U tiles (read once from L2 for up to 512 output columns); the tap segments (split K) of a slice balance the
@@ -234,7 +464,7 @@ int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
 template <int PLANES>
 __global__ void __launch_bounds__(CORR_THREADS, 1)
 corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restrict__ maps, const TcCorrUnit *__restrict__ units,
-               const int *__restrict__ cta_begin, const long long *__restrict__ n0_ptr) {
+               const int *__restrict__ cta_begin, const long long *__restrict__ n0_ptr, int terms) {
   constexpr int STAGES = PLANES == 2 ? 4 : 6;
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -316,7 +546,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
                 for (int sb = 0; sb < NS; ++sb) {
                   const uint64_t x_hi = xk + 16 * k + sdesc[sb], x_lo = x_hi + (STRIP_PLANE >> 4);
                   mma_f16_ss(d0 + dcol[sb], u_hi, x_hi, idesc[sb], acc);
-                  if (PLANES == 2) { mma_f16_ss(d0 + dcol[sb], u_hi, x_lo, idesc[sb], true); mma_f16_ss(d0 + dcol[sb], u_lo, x_hi, idesc[sb], true); }
+                  if (PLANES == 2) { if (terms & 2) mma_f16_ss(d0 + dcol[sb], u_hi, x_lo, idesc[sb], true); if (terms & 4) mma_f16_ss(d0 + dcol[sb], u_lo, x_hi, idesc[sb], true); }
                 }
               }
               mma_commit(&uempty[stage]);
@@ -459,8 +689,9 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 
 // ------------------------------------------------------------------------------------------------ host side
 struct TcPlan {
-  int planes, n_det, B, n_tt;
+  int planes, n_det, B, n_tt, terms;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
+  TsItem *ts_items_dev; int *ts_begin_dev; int n_ts_items, ts_grid, ts_smem, ts_rlo_bytes, ts_ystages;   // resident-R a3
   int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
@@ -527,12 +758,12 @@ static EncodeTiledFn get_encode() {
 }
 
 // fp16 row-major [rows][cols] (cols % 64 == 0), box = 64 columns x 128 rows, 128-byte swizzle
-static bool make_map(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols) {
+static bool make_map(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, int box_rows) {
   EncodeTiledFn enc = get_encode();
   if (!enc) { set_error("stream_create: cuTensorMapEncodeTiled is not available from the driver"); return false; }
   cuuint64_t dims[2] = {cols, rows};
   cuuint64_t strides[1] = {cols * 2};
-  cuuint32_t box[2] = {BK, TILE_M};
+  cuuint32_t box[2] = {BK, (cuuint32_t)box_rows};
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
                    CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
@@ -566,6 +797,8 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
+  p->terms = 0x77;
+  if (const char *t = getenv("LLOID_DEBUG_TERMS")) p->terms = (int)strtol(t, nullptr, 16);   // EXPERIMENT ONLY
   // ---- a2: one tensor map per class; units = (row tile, tap segment, group of <= 4 (detector, column tile) sub-tiles),
   //      dealt to the persistent CTAs in order of decreasing cost
   std::vector<TcCorrClass> cm(classes.size());
@@ -573,7 +806,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   for (size_t ci = 0; ci < classes.size(); ++ci) {
     const CorrClass &c = classes[ci];
     memset(&cm[ci], 0, sizeof(TcCorrClass));
-    if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad, TILE_M)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     const int nseg = tc_k_segments(c.Npad);
     const int kseg = ((c.Npad + nseg - 1) / nseg + BK - 1) / BK * BK;
     struct Sub { int det, c0, w; };
@@ -607,36 +840,75 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
       }
   }
   p->n_cunits = (int)cu.size();
-  // ---- a3: two tensor maps per bank; tiles ordered (bank, template tile, detector, time tile)
+  // ---- a3: tensor maps per bank.  Banks whose concatenated basis axis fits the resident-R kernel (split mode, Kpad <=
+  //      TS_KMAX) become TsItems; the others are tiled (bank, template tile, detector, time tile) for the streaming kernel
   std::vector<TcReconBank> rb(banks.size());
   std::vector<TcReconTile> rt;
+  std::vector<TsItem> ts;
+  std::vector<char> is_ts(banks.size(), 0);
   for (size_t b = 0; b < banks.size(); ++b) {
     const ReconBank &k = banks[b];
     memset(&rb[b], 0, sizeof(TcReconBank));
-    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad) ||
-        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M) ||
+        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M) ||
+        !make_map(&rb[b].mapY64, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TS_NT)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    rb[b].R16 = k.R16;
     rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
+    is_ts[b] = (planes == 2 && k.Kpad <= TS_KMAX && !getenv("LLOID_DEBUG_NO_TS")) ? 1 : 0;
   }
-  long long n_mu = 0;
-  for (const ReconBank &k : banks) n_mu += (long long)((k.M + TILE_M - 1) / TILE_M) * n_det;
-  const int nt = recon_run_tiles(B, n_mu), ntile = (B + TILE_N - 1) / TILE_N;
-  p->n_tt = tc_time_splits(B, n_mu);
-  for (size_t b = 0; b < banks.size(); ++b) {
-    const ReconBank &k = banks[b];
-    for (int m0 = 0; m0 < k.M; m0 += TILE_M)
-      for (int det = 0; det < n_det; ++det)
-        for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
-  }
-  p->n_rtiles = (int)rt.size();
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
+  long long n_mu = 0, n_bm = 0;
+  int nkb_max = 1;
+  for (size_t b = 0; b < banks.size(); ++b) {
+    const long long mt = (banks[b].M + TILE_M - 1) / TILE_M;
+    if (is_ts[b]) { n_bm += mt; nkb_max = std::max(nkb_max, (banks[b].Kpad + BK - 1) / BK); }
+    else n_mu += mt * n_det;
+  }
+  const int nt = recon_run_tiles(B, n_mu), ntile = (B + TILE_N - 1) / TILE_N;
+  p->n_tt = n_mu ? tc_time_splits(B, n_mu) : 2;
+  // resident-R items: one (bank, template tile) per item; split by detector, then by runs of time tiles, until the
+  // persistent grid has a few items per SM
+  const int tiles64 = (B + TS_NT - 1) / TS_NT;
+  const int det_split = (n_bm < 4LL * sms && n_det > 1) ? n_det : 1;
+  int r_time = 1;
+  while (n_bm * det_split * r_time < 2LL * sms && tiles64 / (r_time * 2) >= 2) r_time *= 2;
+  const int nt_run = (tiles64 + r_time - 1) / r_time, n_runs = (tiles64 + nt_run - 1) / nt_run;
+  if (n_bm) p->n_tt = std::max(p->n_tt, 2 * n_runs);
+  for (size_t b = 0; b < banks.size(); ++b) {
+    const ReconBank &k = banks[b];
+    for (int m0 = 0; m0 < k.M; m0 += TILE_M) {
+      if (is_ts[b]) {
+        const int nd = n_det / det_split;
+        for (int dg = 0; dg < det_split; ++dg)
+          for (int r = 0; r < n_runs; ++r)
+            ts.push_back({(int)b, m0, dg * nd, nd, r * nt_run * TS_NT, std::min(nt_run, tiles64 - r * nt_run), r});
+      } else {
+        for (int det = 0; det < n_det; ++det)
+          for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
+      }
+    }
+  }
+  p->n_ts_items = (int)ts.size();
+  p->ts_grid = std::max(1, std::min(p->n_ts_items, sms));
+  p->ts_rlo_bytes = 2 * nkb_max * TILE_BYTES;
+  p->ts_ystages = std::min(TS_MAX_YSTAGES, (232448 - 1024 - 256 - p->ts_rlo_bytes - TS_REC_BYTES) / TS_YSTAGE);
+  p->ts_smem = 1024 + p->ts_rlo_bytes + p->ts_ystages * TS_YSTAGE + TS_REC_BYTES + 256;
+  p->n_rtiles = (int)rt.size();
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
   std::vector<int> cbegin, rbegin;
   lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1] + u.nt[2] + u.nt[3]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
   lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * ((rb[t.bank].Kpad + BK - 1) / BK + 1); }, rbegin);
-  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+  std::vector<int> tsbegin;
+  // cost in cycles: per tile the larger of the MMA stream (6 MMAs of 32 cycles per 16 of K) and the peak-search epilogue,
+  // plus the once-per-item load of the template tile's R
+  lpt_assign(ts, p->ts_grid, [&](const TsItem &t) {
+    const long long kp = rb[t.bank].Kpad;
+    return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 192, 450) + kp * 16 + 1500; }, tsbegin);
+  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->ts_items_dev, ts) ||
+      !plan_upload(p, &p->ts_begin_dev, tsbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   const int rstages = planes == 2 ? 2 : 4;
@@ -650,6 +922,10 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     e = cudaFuncSetAttribute(recon_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(corr_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->corr_smem);
   }
+  if (e == cudaSuccess && p->n_ts_items) {
+    if (p->ts_ystages < 2) { set_error("stream_create: no shared memory left for the Y stages of the resident-R kernel"); tc_plan_destroy(p); return LLOID_EINVAL; }
+    e = cudaFuncSetAttribute(recon_ts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p->ts_smem);
+  }
   if (e != cudaSuccess) { set_error("stream_create: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); tc_plan_destroy(p); return LLOID_ECUDA; }
   *out = p;
   return LLOID_OK;
@@ -658,19 +934,26 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
   if (p->n_cunits == 0) return cudaSuccess;
   if (p->planes == 2)
-    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
+    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0, p->terms);
   else
-    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
+    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0, p->terms);
   return cudaGetLastError();
 }
 
+int tc_plan_n_tt(const TcPlan *p) { return p->n_tt; }
+int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_ts_items ? 1 : 0); }
+
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
+  if (p->n_ts_items)
+    recon_ts_kernel<<<p->ts_grid, TS_THREADS, p->ts_smem, st>>>(p->rbanks_dev, p->ts_items_dev, p->ts_begin_dev, p->n_det, p->B, partial, Mtot,
+                                                              p->n_tt, snr_debug, debug_bank, p->ts_rlo_bytes, p->ts_ystages);
+  if (p->n_rtiles == 0) return cudaGetLastError();
   if (p->planes == 2)
     recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
+                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank, p->terms);
   else
     recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
+                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank, p->terms);
   return cudaGetLastError();
 }
 

@@ -114,6 +114,7 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
                             const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st);
 cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
+cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st);
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
                             lloid_peak *peaks, long long *n0, int B, cudaStream_t st);
 
@@ -124,6 +125,8 @@ int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel f
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
                    const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes);
 void tc_plan_destroy(TcPlan *p);
+int tc_plan_n_tt(const TcPlan *p);              // partial peaks per template and detector the a3 kernels write
+int tc_plan_recon_launches(const TcPlan *p);    // 1 or 2: streaming kernel and / or resident-R kernel
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st);
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank,
                             cudaStream_t st);

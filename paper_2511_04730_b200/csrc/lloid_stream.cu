@@ -326,18 +326,19 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   CK(dev_upload(s, &s->items_dev, items));
   CK(dev_upload(s, &s->uprows_dev, uprows));
   CK(dev_upload(s, &s->rbanks_dev, s->rbanks));
-  long long n_mu = 0;
-  for (const lloid_bank *bk : s->banks) n_mu += (long long)((bk->M + 127) / 128) * n_det;
-  s->n_tt = (s->precision == LLOID_PREC_FP32_FFMA) ? (B + 63) / 64 : tc_time_splits(B, n_mu);
-  CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
+  s->n_tt = (B + 63) / 64;
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
   if (s->precision != LLOID_PREC_FP32_FFMA) {
     int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
+    s->n_tt = tc_plan_n_tt(s->tc);                 // partial peaks per template: the larger of the two a3 kernels' splits
     s->work[0] *= (planes == 2 ? 3 : 1);
     s->work[1] *= (planes == 2 ? 3 : 1);
   }
+  // partial-peak slots a kernel never writes hold p = -3 (below every real partial, finalize ignores them)
+  CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
+  CK(launch_fill_partial(s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt, s->st));
   CK(cudaDeviceSynchronize());
   *out = s;
   return LLOID_OK;
@@ -416,7 +417,7 @@ extern "C" int lloid_state_reset(lloid_stream *s) {
 
 extern "C" int64_t lloid_stream_samples_pushed(const lloid_stream *s) { return s ? s->n0_host : -1; }
 extern "C" int32_t lloid_stream_total_templates(const lloid_stream *s) { return s ? s->Mtot : -1; }
-extern "C" int32_t lloid_stream_launches_per_push(const lloid_stream *s) { return s ? 5 : -1; }
+extern "C" int32_t lloid_stream_launches_per_push(const lloid_stream *s) { return s ? 4 + (s->tc ? tc_plan_recon_launches(s->tc) : 1) : -1; }
 extern "C" int lloid_stream_work_per_push(const lloid_stream *s, double out[8]) {
   if (!s || !out) { set_error("work_per_push: NULL argument"); return LLOID_EINVAL; }
   for (int i = 0; i < 8; ++i) out[i] = s->work[i];

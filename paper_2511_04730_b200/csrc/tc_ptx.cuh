@@ -78,6 +78,25 @@ __device__ __forceinline__ void tmem_ld_32x32(uint32_t taddr, uint32_t (&v)[32])
       : "r"(taddr)
       : "memory");
 }
+// 32 lanes x 16 consecutive columns
+__device__ __forceinline__ void tmem_ld_32x16(uint32_t taddr, uint32_t (&v)[16]) {
+  asm volatile(
+      "tcgen05.ld.sync.aligned.32x32b.x16.b32 "
+      "{%0, %1, %2, %3, %4, %5, %6, %7, %8, %9, %10, %11, %12, %13, %14, %15}, [%16];"
+      : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7]), "=r"(v[8]),
+        "=r"(v[9]), "=r"(v[10]), "=r"(v[11]), "=r"(v[12]), "=r"(v[13]), "=r"(v[14]), "=r"(v[15])
+      : "r"(taddr)
+      : "memory");
+}
+// registers -> TMEM: thread t of the warp writes 8 consecutive 32-bit columns of lane (base lane + t).  Used to place a
+// 16-bit A operand in tensor memory: row m = lane m, element k in column k/2 (low half = even k), PTX ISA "tcgen05.mma
+// A matrix in tensor memory" (two 16-bit elements per 32-bit column).
+__device__ __forceinline__ void tmem_st_32x8(uint32_t taddr, const uint32_t (&v)[8]) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1, %2, %3, %4, %5, %6, %7, %8};" ::"r"(taddr), "r"(v[0]), "r"(v[1]),
+               "r"(v[2]), "r"(v[3]), "r"(v[4]), "r"(v[5]), "r"(v[6]), "r"(v[7])
+               : "memory");
+}
+__device__ __forceinline__ void tmem_st_wait() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_ld_wait() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 
 // ------------------------------------------------------------------------------------------------ descriptors
@@ -106,6 +125,14 @@ __device__ __forceinline__ void mma_f16_ss(uint32_t d_tmem, uint64_t a_desc, uin
       ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate)
       : "memory");
 }
+// D[tmem] (+)= A[tmem] * B[smem]: the A operand (M = 128 rows = 128 lanes, 16-bit elements packed two per column) is read
+// from tensor memory, so only B costs shared-memory bandwidth
+__device__ __forceinline__ void mma_f16_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, bool accumulate) {
+  asm volatile(
+      "{ .reg .pred p; setp.ne.b32 p, %4, 0; tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p; }"
+      ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"((uint32_t)accumulate)
+      : "memory");
+}
 // same with the accumulate flag known at compile time (no setp from a register): the issuing thread is on the
 // critical path of the tensor pipe, every instruction it saves counts
 __device__ __forceinline__ void mma_f16_ss_acc(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc) {
@@ -119,6 +146,13 @@ __device__ __forceinline__ void mma_commit(uint64_t *bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
 }
 
+// |z|^2 of two samples with packed fp32x2 arithmetic: p = fma(im, im, re * re), both round-to-nearest (identical to the
+// scalar __fmaf_rn(im, im, __fmul_rn(re, re)))
+__device__ __forceinline__ void abs2_x2(float re0, float re1, float im0, float im1, float &p0, float &p1) {
+  asm("{ .reg .b64 r, i, t; mov.b64 r, {%2, %3}; mov.b64 i, {%4, %5}; mul.rn.f32x2 t, r, r; fma.rn.f32x2 t, i, i, t; mov.b64 {%0, %1}, t; }"
+      : "=f"(p0), "=f"(p1)
+      : "f"(re0), "f"(re1), "f"(im0), "f"(im1));
+}
 __device__ __forceinline__ bool elect_one() {
   uint32_t pred;
   asm volatile("{ .reg .pred p; elect.sync _|p, 0xffffffff; selp.u32 %0, 1, 0, p; }" : "=r"(pred));
