@@ -3,6 +3,8 @@
 // they are latency/HBM-bound stages, not contractions.
 #include <cmath>
 
+#include <cuda_fp8.h>
+
 #include "lloid_internal.h"
 
 namespace lloid {
@@ -141,7 +143,12 @@ __device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_strid
   } else {
     __half hi16 = __float2half_rn(v);
     reinterpret_cast<__half *>(yup)[o] = hi16;
-    if (HALF_PLANES == 2) reinterpret_cast<__half *>(yup)[o + plane_stride] = __float2half_rn(v - __half2float(hi16));
+    if (HALF_PLANES == 2) {
+      // correction plane: 16 bits = { e5m2(4 Y_lo), e5m2(Y_hi / 256) }, B operand of the fp8 MMA of a3
+      const float hf = __half2float(hi16);
+      reinterpret_cast<unsigned short *>(yup)[o + plane_stride] =
+          __nv_cvt_float2_to_fp8x2(make_float2((v - hf) * 4.f, hf * (1.f / 256.f)), __NV_SATFINITE, __NV_E5M2);
+    }
   }
 }
 

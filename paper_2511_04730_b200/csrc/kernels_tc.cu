@@ -9,10 +9,13 @@
 #include <cuda.h>
 
 #include <algorithm>
+#include <cstdio>
 #include <cstdlib>
 #include <cstring>
 #include <queue>
 #include <type_traits>
+
+#include <cuda_fp8.h>
 
 #include "lloid_internal.h"
 #include "tc_ptx.cuh"
@@ -50,7 +53,7 @@ template <int PLANES>
 __global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                 int n_det, int B,
-                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank, int terms) {
+                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank) {
   constexpr int STAGES = PLANES == 2 ? 2 : 4;
   constexpr int STAGE_BYTES = 3 * PLANES * TILE_BYTES;        // Rre, Rim, Y per plane
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -95,14 +98,14 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N);
-      int stage = 0; uint32_t phase = 0; int it = 0;
-      for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
-        const TcReconTile tl = tiles[ti];
-        const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
-        for (int tt = 0; tt < tl.nt; ++tt, ++it) {
+    // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers),
+    // one elected lane issues the MMAs of a K block and the commits
+    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N), idesc8 = idesc_f8_f32(TILE_M, TILE_N);
+    int stage = 0; uint32_t phase = 0; int it = 0;
+    for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
+      const TcReconTile tl = tiles[ti];
+      const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
+      for (int tt = 0; tt < tl.nt; ++tt, ++it) {
         const int buf = it & 1;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
@@ -113,25 +116,29 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           // one base descriptor per stage; every operand tile / K step is a constant added to its 16-byte address field
           const uint64_t db = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
           const int nk = min(BK / 16, (Kpad - kb * BK) / 16);       // K is padded to 16, the last 64-wide box is zero-filled
+          if (elect_one()) {
 #pragma unroll
-          for (int k = 0; k < BK / 16; ++k) {
-            if (k >= nk) break;
-            const bool acc = (kb | k) != 0;
-            const uint64_t re_hi = db + ((0 * TILE_BYTES + k * 32) >> 4), im_hi = db + ((1 * TILE_BYTES + k * 32) >> 4),
-                           y_hi = db + ((2 * TILE_BYTES + k * 32) >> 4);
-            mma_f16_ss(d_re, re_hi, y_hi, idesc, acc);
-            mma_f16_ss(d_im, im_hi, y_hi, idesc, acc);
-            if (PLANES == 2) {
-              const uint64_t re_lo = db + ((3 * TILE_BYTES + k * 32) >> 4), im_lo = db + ((4 * TILE_BYTES + k * 32) >> 4),
-                             y_lo = db + ((5 * TILE_BYTES + k * 32) >> 4);
-              if (terms & 0x20) { mma_f16_ss(d_re, re_hi, y_lo, idesc, true); mma_f16_ss(d_im, im_hi, y_lo, idesc, true); }
-              if (terms & 0x40) { mma_f16_ss(d_re, re_lo, y_hi, idesc, true); mma_f16_ss(d_im, im_lo, y_hi, idesc, true); }
+            for (int k = 0; k < BK / 16; ++k) {
+              if (k >= nk) break;
+              const bool acc = (kb | k) != 0;
+              const uint64_t re_hi = db + ((0 * TILE_BYTES + k * 32) >> 4), im_hi = db + ((1 * TILE_BYTES + k * 32) >> 4),
+                             y_hi = db + ((2 * TILE_BYTES + k * 32) >> 4);
+              mma_f16_ss(d_re, re_hi, y_hi, idesc, acc);
+              mma_f16_ss(d_im, im_hi, y_hi, idesc, acc);
+              if (PLANES == 2) {
+                // the correction planes: 32 bytes = 16 of K as (e4m3, e4m3) x (e5m2, e5m2) pairs -> one fp8 MMA adds both
+                // cross terms R_hi Y_lo + R_lo Y_hi
+                const uint64_t re_8 = db + ((3 * TILE_BYTES + k * 32) >> 4), im_8 = db + ((4 * TILE_BYTES + k * 32) >> 4),
+                               y_8 = db + ((5 * TILE_BYTES + k * 32) >> 4);
+                mma_f8_ss(d_re, re_8, y_8, idesc8, true);
+                mma_f8_ss(d_im, im_8, y_8, idesc8, true);
+              }
             }
+            mma_commit(&empty[stage]);
+            if (kb == nkb - 1) mma_commit(&tfull[buf]);
           }
-          mma_commit(&empty[stage]);
+          __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-        mma_commit(&tfull[buf]);
         }
       }
     }
@@ -280,51 +287,54 @@ recon_ts_kernel(const TcReconBank *__restrict__ banks, const TsItem *__restrict_
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer
-    if (lane == 0) {
-      constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TS_NT);
-      int stage = 0; uint32_t phase = 0; int t_it = 0;
-      for (int ii = i_begin; ii < i_end; ++ii) {
-        const TsItem it = items[ii];
-        const int Kpad = banks[it.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
-        const uint32_t ip = (uint32_t)(ii - i_begin) & 1;
-        mbar_wait(rfull, ip);
-        mbar_wait(rlofull, ip);
+    // ===== MMA issuer.  The whole warp runs the loops (uniform control flow and data: descriptors stay in uniform
+    // registers); one elected lane issues the MMAs of a K block and the commits.
+    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TS_NT), idesc8 = idesc_f8_f32(TILE_M, TS_NT);
+    int stage = 0; uint32_t phase = 0; int t_it = 0;
+    for (int ii = i_begin; ii < i_end; ++ii) {
+      const TsItem it = items[ii];
+      const int Kpad = banks[it.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
+      const uint32_t ip = (uint32_t)(ii - i_begin) & 1;
+      mbar_wait(rfull, ip);
+      mbar_wait(rlofull, ip);
+      tc_fence_after_sync();
+      const uint32_t a_re0 = tmem + 256, a_im0 = a_re0 + (Kpad >> 1);
+      const uint64_t rl_re0 = desc_kmajor_sw128(smem_u32(rlo)), rl_im0 = desc_kmajor_sw128(smem_u32(rlo + nkb * TILE_BYTES));
+      const int ntile = it.ndet * it.nt;
+      for (int tl = 0; tl < ntile; ++tl, ++t_it) {
+        const int buf = t_it & 1;
+        mbar_wait(&tempty[buf], ((t_it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
-        const uint32_t a_re0 = tmem + 256, a_im0 = a_re0 + (Kpad >> 1);
-        const uint64_t rl_re0 = desc_kmajor_sw128(smem_u32(rlo)), rl_im0 = desc_kmajor_sw128(smem_u32(rlo + nkb * TILE_BYTES));
-        const int ntile = it.ndet * it.nt;
-        for (int tl = 0; tl < ntile; ++tl, ++t_it) {
-          const int buf = t_it & 1;
-          mbar_wait(&tempty[buf], ((t_it >> 1) & 1) ^ 1);
+        const uint32_t d_re = tmem + buf * 128, d_im = d_re + 64;
+        for (int kb = 0; kb < nkb; ++kb) {
+          mbar_wait(&yfull[stage], phase);
           tc_fence_after_sync();
-          const uint32_t d_re = tmem + buf * 128, d_im = d_re + 64;
-          for (int kb = 0; kb < nkb; ++kb) {
-            mbar_wait(&yfull[stage], phase);
-            tc_fence_after_sync();
-            const uint64_t yd = desc_kmajor_sw128(smem_u32(ybuf + stage * TS_YSTAGE));
-            const int nk = min(BK / 16, (Kpad - kb * BK) / 16);
+          const uint64_t yd = desc_kmajor_sw128(smem_u32(ybuf + stage * TS_YSTAGE));
+          const int nk = min(BK / 16, (Kpad - kb * BK) / 16);
+          const uint32_t ks0 = (uint32_t)(kb * (BK / 16)) * 8;
+          const uint64_t off0 = (uint64_t)((kb * TILE_BYTES) >> 4);
+          if (elect_one()) {
 #pragma unroll
             for (int k = 0; k < BK / 16; ++k) {
               if (k >= nk) break;
               const bool acc = (kb | k) != 0;
-              const uint32_t ks = (uint32_t)(kb * (BK / 16) + k) * 8;            // 16 fp16 of K = 8 TMEM columns
+              const uint32_t ks = ks0 + k * 8;                                  // 16 fp16 of K = 8 TMEM columns
               const uint64_t y_hi = yd + 2 * k, y_lo = y_hi + (TS_YTILE >> 4);
-              const uint64_t off = (uint64_t)((kb * TILE_BYTES + k * 32) >> 4);
+              const uint64_t off = off0 + 2 * k;
               mma_f16_ts(d_re, a_re0 + ks, y_hi, idesc, acc);
               mma_f16_ts(d_im, a_im0 + ks, y_hi, idesc, acc);
-              mma_f16_ts(d_re, a_re0 + ks, y_lo, idesc, true);
-              mma_f16_ts(d_im, a_im0 + ks, y_lo, idesc, true);
-              mma_f16_ss(d_re, rl_re0 + off, y_hi, idesc, true);
-              mma_f16_ss(d_im, rl_im0 + off, y_hi, idesc, true);
+              mma_f8_ss(d_re, rl_re0 + off, y_lo, idesc8, true);                  // both cross terms in one fp8 MMA
+              mma_f8_ss(d_im, rl_im0 + off, y_lo, idesc8, true);
             }
             mma_commit(&yempty[stage]);
-            if (++stage == n_ys) { stage = 0; phase ^= 1; }
+            if (kb == nkb - 1) mma_commit(&tfull[buf]);
           }
-          mma_commit(&tfull[buf]);
+          __syncwarp();
+          if (++stage == n_ys) { stage = 0; phase ^= 1; }
         }
-        mma_commit(rdone);
       }
+      if (elect_one()) mma_commit(rdone);
+      __syncwarp();
     }
   } else {
     // ===== epilogue warps (8): thread = template (TMEM lane) x one half (32 samples) of the tile; they also place R_hi of
@@ -464,7 +474,7 @@ int tc_k_segments(int Npad) { return (Npad + KSEG_MAX - 1) / KSEG_MAX; }
 template <int PLANES>
 __global__ void __launch_bounds__(CORR_THREADS, 1)
 corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restrict__ maps, const TcCorrUnit *__restrict__ units,
-               const int *__restrict__ cta_begin, const long long *__restrict__ n0_ptr, int terms) {
+               const int *__restrict__ cta_begin, const long long *__restrict__ n0_ptr) {
   constexpr int STAGES = PLANES == 2 ? 4 : 6;
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
@@ -508,59 +518,63 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
     }
   } else if (warp == 1) {
     // ===== MMA issuer.  Descriptors differ only in their 14-bit address field (16-byte units): one 64-bit add each.
-    if (lane == 0) {
-      int stage = 0; uint32_t phase = 0; int it = 0, chunk_it = 0;
-      for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
-        const TcCorrUnit *u = &units[ui];
-        const int nsub = u->nsub, k0 = u->k0, k1 = u->k1;
-        uint32_t idesc[MAX_SUB], dcol[MAX_SUB], sdesc[MAX_SUB];
+    // The whole warp runs the loops (uniform control flow: descriptors stay in uniform registers); one elected lane
+    // issues the MMAs of a 64-tap block and the commits.
+    int stage = 0; uint32_t phase = 0; int it = 0, chunk_it = 0;
+    for (int ui = cta_begin[blockIdx.x]; ui < cta_begin[blockIdx.x + 1]; ++ui, ++it) {
+      const TcCorrUnit *u = &units[ui];
+      const int nsub = u->nsub, k0 = u->k0, k1 = u->k1;
+      uint32_t idesc[MAX_SUB], dcol[MAX_SUB], sdesc[MAX_SUB];
 #pragma unroll
-        for (int sb = 0; sb < MAX_SUB; ++sb) {
-          idesc[sb] = idesc_f16_f32(TILE_M, sb < nsub ? u->nt[sb] : 16);
-          dcol[sb] = sb < nsub ? u->tcol[sb] : 0;
-          sdesc[sb] = sb < nsub ? (uint32_t)(u->soff[sb] >> 4) : 0;
-        }
-        const int buf = it & 1;
-        mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
-        tc_fence_after_sync();
-        const uint32_t d0 = tmem + buf * UNIT_N;
-        // the chunk / k loops, specialised on the number of sub-tiles so the single issuing thread runs straight-line code
-        auto issue = [&](auto ns_tag) {
-          constexpr int NS = decltype(ns_tag)::value;
-          for (int kc = k0; kc < k1; kc += KS, ++chunk_it) {
-            const int sbuf = chunk_it & 1;
-            mbar_wait(&sfull[sbuf], (chunk_it >> 1) & 1);
+      for (int sb = 0; sb < MAX_SUB; ++sb) {
+        idesc[sb] = idesc_f16_f32(TILE_M, sb < nsub ? u->nt[sb] : 16);
+        dcol[sb] = sb < nsub ? u->tcol[sb] : 0;
+        sdesc[sb] = sb < nsub ? (uint32_t)(u->soff[sb] >> 4) : 0;
+      }
+      const int buf = it & 1;
+      mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
+      tc_fence_after_sync();
+      const uint32_t d0 = tmem + buf * UNIT_N;
+      // the chunk / k loops, specialised on the number of sub-tiles so the issuing lane runs straight-line code
+      auto issue = [&](auto ns_tag) {
+        constexpr int NS = decltype(ns_tag)::value;
+        for (int kc = k0; kc < k1; kc += KS, ++chunk_it) {
+          const int sbuf = chunk_it & 1;
+          mbar_wait(&sfull[sbuf], (chunk_it >> 1) & 1);
+          tc_fence_after_sync();
+          const uint64_t xd = desc_kmajor_nosw(smem_u32(strips + sbuf * PLANES * STRIP_PLANE), 128, 128);
+          const int kend = min(kc + KS, k1);
+          for (int kb = kc; kb < kend; kb += BK) {
+            mbar_wait(&ufull[stage], phase);
             tc_fence_after_sync();
-            const uint64_t xd = desc_kmajor_nosw(smem_u32(strips + sbuf * PLANES * STRIP_PLANE), 128, 128);
-            const int kend = min(kc + KS, k1);
-            for (int kb = kc; kb < kend; kb += BK) {
-              mbar_wait(&ufull[stage], phase);
-              tc_fence_after_sync();
-              const uint64_t ud = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
-              const uint64_t xk = xd + (uint64_t)(kb - kc);              // 16 B per tap
+            const uint64_t ud = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
+            const uint64_t xk = xd + (uint64_t)(kb - kc);              // 16 B per tap
+            if (elect_one()) {
 #pragma unroll
               for (int k = 0; k < BK / 16; ++k) {
                 const bool acc = (kb > k0) || (k > 0);
                 const uint64_t u_hi = ud + 2 * k, u_lo = u_hi + (TILE_BYTES >> 4);
 #pragma unroll
                 for (int sb = 0; sb < NS; ++sb) {
-                  const uint64_t x_hi = xk + 16 * k + sdesc[sb], x_lo = x_hi + (STRIP_PLANE >> 4);
+                  const uint64_t x_hi = xk + 16 * k + sdesc[sb], x_8 = x_hi + (STRIP_PLANE >> 4);
                   mma_f16_ss(d0 + dcol[sb], u_hi, x_hi, idesc[sb], acc);
-                  if (PLANES == 2) { if (terms & 2) mma_f16_ss(d0 + dcol[sb], u_hi, x_lo, idesc[sb], true); if (terms & 4) mma_f16_ss(d0 + dcol[sb], u_lo, x_hi, idesc[sb], true); }
+                  // correction planes: 16 taps = 32 bytes of (e4m3, e4m3) x (e5m2, e5m2) pairs: one fp8 MMA adds U_hi x_lo + U_lo x_hi
+                  if (PLANES == 2) mma_f8_ss(d0 + dcol[sb], u_lo, x_8, idesc[sb] | (1u << 10), true);
                 }
               }
               mma_commit(&uempty[stage]);
-              if (++stage == STAGES) { stage = 0; phase ^= 1; }
+              if (kb + BK >= kend) mma_commit(&sempty[sbuf]);
+              if (kb + BK >= k1) mma_commit(&tfull[buf]);
             }
-            mma_commit(&sempty[sbuf]);
+            __syncwarp();
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
-        };
-        if (nsub == 1) issue(std::integral_constant<int, 1>());
-        else if (nsub == 2) issue(std::integral_constant<int, 2>());
-        else if (nsub == 3) issue(std::integral_constant<int, 3>());
-        else issue(std::integral_constant<int, 4>());
-        mma_commit(&tfull[buf]);
-      }
+        }
+      };
+      if (nsub == 1) issue(std::integral_constant<int, 1>());
+      else if (nsub == 2) issue(std::integral_constant<int, 2>());
+      else if (nsub == 3) issue(std::integral_constant<int, 3>());
+      else issue(std::integral_constant<int, 4>());
     }
   } else if (warp >= 6 && warp < 10) {
     // ===== strip builders (128 threads): stage the strain windows of a unit, then build its strips chunk by chunk
@@ -606,13 +620,17 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
             float v[8];
 #pragma unroll
             for (int i = 0; i < 8; ++i) v[i] = xs[e + i];
-            __half2 h[4], l[4];
+            __half2 h[4];
+            uint32_t l[4];
 #pragma unroll
             for (int i = 0; i < 4; ++i) {
               h[i] = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
               if (PLANES == 2) {
-                float2 bb = __half22float2(h[i]);
-                l[i] = __floats2half2_rn(v[2 * i] - bb.x, v[2 * i + 1] - bb.y);
+                // correction strip: per tap 16 bits = { e5m2(4 x_lo), e5m2(x_hi / 256) }
+                const float2 bb = __half22float2(h[i]);
+                const uint32_t p0 = __nv_cvt_float2_to_fp8x2(make_float2((v[2 * i] - bb.x) * 4.f, bb.x * (1.f / 256.f)), __NV_SATFINITE, __NV_E5M2);
+                const uint32_t p1 = __nv_cvt_float2_to_fp8x2(make_float2((v[2 * i + 1] - bb.y) * 4.f, bb.y * (1.f / 256.f)), __NV_SATFINITE, __NV_E5M2);
+                l[i] = p0 | (p1 << 16);
               }
             }
             *reinterpret_cast<uint4 *>(dst + (size_t)e * 16) = *reinterpret_cast<uint4 *>(h);
@@ -689,7 +707,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 
 // ------------------------------------------------------------------------------------------------ host side
 struct TcPlan {
-  int planes, n_det, B, n_tt, terms;
+  int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
   TsItem *ts_items_dev; int *ts_begin_dev; int n_ts_items, ts_grid, ts_smem, ts_rlo_bytes, ts_ystages;   // resident-R a3
   int *rbegin_dev, *cbegin_dev;
@@ -797,8 +815,6 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
-  p->terms = 0x77;
-  if (const char *t = getenv("LLOID_DEBUG_TERMS")) p->terms = (int)strtol(t, nullptr, 16);   // EXPERIMENT ONLY
   // ---- a2: one tensor map per class; units = (row tile, tap segment, group of <= 4 (detector, column tile) sub-tiles),
   //      dealt to the persistent CTAs in order of decreasing cost
   std::vector<TcCorrClass> cm(classes.size());
@@ -924,7 +940,11 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   }
   if (e == cudaSuccess && p->n_ts_items) {
     if (p->ts_ystages < 2) { set_error("stream_create: no shared memory left for the Y stages of the resident-R kernel"); tc_plan_destroy(p); return LLOID_EINVAL; }
-    e = cudaFuncSetAttribute(recon_ts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, p->ts_smem);
+    // the limit is per function and device, not per stream: always opt in to the device maximum so that streams with
+    // different resident-R footprints can coexist in one process
+    int optin = 0;
+    cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
+    e = cudaFuncSetAttribute(recon_ts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(optin, p->ts_smem));
   }
   if (e != cudaSuccess) { set_error("stream_create: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); tc_plan_destroy(p); return LLOID_ECUDA; }
   *out = p;
@@ -934,9 +954,9 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
   if (p->n_cunits == 0) return cudaSuccess;
   if (p->planes == 2)
-    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0, p->terms);
+    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
   else
-    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0, p->terms);
+    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
   return cudaGetLastError();
 }
 
@@ -947,13 +967,24 @@ cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *sn
   if (p->n_ts_items)
     recon_ts_kernel<<<p->ts_grid, TS_THREADS, p->ts_smem, st>>>(p->rbanks_dev, p->ts_items_dev, p->ts_begin_dev, p->n_det, p->B, partial, Mtot,
                                                               p->n_tt, snr_debug, debug_bank, p->ts_rlo_bytes, p->ts_ystages);
-  if (p->n_rtiles == 0) return cudaGetLastError();
+  {
+    cudaError_t e0 = cudaGetLastError();
+    if (e0 != cudaSuccess || p->n_rtiles == 0) {
+      if (e0 != cudaSuccess) {
+        cudaFuncAttributes fa; memset(&fa, 0, sizeof(fa));
+        cudaFuncGetAttributes(&fa, recon_ts_kernel);
+        int dev = -1; cudaGetDevice(&dev);
+        fprintf(stderr, "lloid: recon_ts_kernel launch failed: grid %d smem %d rlo %d ystages %d items %d: %s; func maxDyn %d static %zu regs %d dev %d\n", p->ts_grid, p->ts_smem, p->ts_rlo_bytes, p->ts_ystages, p->n_ts_items, cudaGetErrorString(e0), fa.maxDynamicSharedSizeBytes, fa.sharedSizeBytes, fa.numRegs, dev);
+      }
+      return e0;
+    }
+  }
   if (p->planes == 2)
     recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank, p->terms);
+                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
   else
     recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank, p->terms);
+                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
   return cudaGetLastError();
 }
 

@@ -7,6 +7,8 @@
 #include <cstring>
 #include <new>
 
+#include <cuda_fp8.h>
+
 #include "lloid_internal.h"
 
 namespace lloid {
@@ -165,7 +167,14 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
       float v = Rh[i] * b->r_scale;
       __half h = __float2half_rn(v);
       R16[i] = h;
-      if (b->r_planes == 2) R16[Rh.size() + i] = __float2half_rn(v - __half2float(h));
+      if (b->r_planes == 2) {
+        // correction plane: 16 bits = { e4m3(R_hi / 4), e4m3(256 R_lo) }, the A operand of the one
+        // fp8 MMA that adds R_hi Y_lo + R_lo Y_hi (its B operand is the matching { e5m2(4 Y_lo), e5m2(Y_hi / 256) })
+        const float hf = __half2float(h);
+        const unsigned lo8 = __nv_cvt_float_to_fp8(hf * 0.25f, __NV_SATFINITE, __NV_E4M3);
+        const unsigned hi8 = __nv_cvt_float_to_fp8((v - hf) * 256.f, __NV_SATFINITE, __NV_E4M3);
+        R16[Rh.size() + i] = __ushort_as_half((unsigned short)(lo8 | (hi8 << 8)));
+      }
     }
     e = cudaMalloc(&b->dR16, R16.size() * sizeof(__half));
     if (e != cudaSuccess) { set_error("bank_create: cudaMalloc R: %s", cudaGetErrorString(e)); lloid_bank_destroy(b); return LLOID_ENOMEM; }

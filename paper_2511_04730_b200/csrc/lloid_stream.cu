@@ -8,6 +8,8 @@
 #include <new>
 #include <tuple>
 
+#include <cuda_fp8.h>
+
 #include "lloid_internal.h"
 
 using namespace lloid;
@@ -223,7 +225,13 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       for (size_t i = 0; i < U.size(); ++i) {
         float v = U[i] * sc; __half h = __float2half_rn(v);
         U16[i] = h;
-        if (planes == 2) U16[U.size() + i] = __float2half_rn(v - __half2float(h));
+        if (planes == 2) {
+          // correction plane: per tap 16 bits = { e4m3(U_hi / 4), e4m3(256 U_lo) }
+          const float hf = __half2float(h);
+          const unsigned lo8 = __nv_cvt_float_to_fp8(hf * 0.25f, __NV_SATFINITE, __NV_E4M3);
+          const unsigned hi8 = __nv_cvt_float_to_fp8((v - hf) * 256.f, __NV_SATFINITE, __NV_E4M3);
+          U16[U.size() + i] = __ushort_as_half((unsigned short)(lo8 | (hi8 << 8)));
+        }
       }
       __half *p; CK(dev_upload(s, &p, U16)); cc.U16 = p;
     }
@@ -333,8 +341,8 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
     s->n_tt = tc_plan_n_tt(s->tc);                 // partial peaks per template: the larger of the two a3 kernels' splits
-    s->work[0] *= (planes == 2 ? 3 : 1);
-    s->work[1] *= (planes == 2 ? 3 : 1);
+    s->work[0] *= (planes == 2 ? 2 : 1);           // split mode: two MMAs per product in a2 (U_hi x, U_lo x) and in a3
+    s->work[1] *= (planes == 2 ? 2 : 1);           // (fp16 R_hi Y_hi + one fp8 MMA carrying both cross terms)
   }
   // partial-peak slots a kernel never writes hold p = -3 (below every real partial, finalize ignores them)
   CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
@@ -361,23 +369,28 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   }
   auto mark = [&](int i) { if (s->stage_timing) cudaEventRecord(ev[i], s->st); };
   mark(0);
+  const char *where = "a1 decimate";
   cudaError_t e = launch_decimate(s->dec, strain, s->n0_dev, s->st);
   mark(1);
   if (e == cudaSuccess) {
+    where = "a2 correlate";
     if (s->tc) e = tc_launch_corr(s->tc, s->n0_dev, s->st);
     else e = launch_corr_ffma(s->classes_dev, s->tiles_dev, s->n_tiles, s->n_det, s->n0_dev, s->st);
   }
   mark(2);
+  if (e == cudaSuccess) where = "a4 upsample";
   if (e == cudaSuccess)
     e = launch_upsample(s->items_dev, s->uprows_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
                         s->n0_dev, s->up_planes, s->taps2, s->st);
   mark(3);
   if (e == cudaSuccess) {
+    where = "a3 reconstruct";
     if (s->tc) e = tc_launch_recon(s->tc, s->partial_dev, s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
     else e = launch_recon_ffma(s->rbanks_dev, (int)s->banks.size(), s->max_mtiles, s->n_det, s->B, s->partial_dev,
                                s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
   }
   mark(4);
+  if (e == cudaSuccess) where = "a5 finalize";
   if (e == cudaSuccess)
     e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->st);
   mark(5);
@@ -386,7 +399,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
     // kernels already enqueued have appended to the rings while the stream clock did not advance: the state is
     // inconsistent, so the stream refuses further pushes (LLOID_ESTATE) until lloid_state_reset
     s->failed = true;
-    set_error("stream_push: launch failed: %s (stream needs lloid_state_reset)", cudaGetErrorString(e)); return LLOID_ECUDA;
+    set_error("stream_push: launch of %s failed: %s (stream needs lloid_state_reset)", where, cudaGetErrorString(e)); return LLOID_ECUDA;
   }
   s->n0_host += s->B;
   return LLOID_OK;
