@@ -23,21 +23,27 @@
 namespace lloid {
 using namespace ptx;
 
-static constexpr int RECON_THREADS = 320;    // a3: warps 0 TMA, 1 MMA, 2-9 epilogue
+static constexpr int EPI_THREADS = 512;      // a3: 16 epilogue warps
+static constexpr int RECON_THREADS = 64 + EPI_THREADS;   // a3: warps 0 TMA, 1 MMA, 2-17 epilogue
+static constexpr int PK_CHUNK = 4;           // samples per peak-search chunk
+static constexpr int REC_BYTES = EPI_THREADS * PK_CHUNK * 8;   // saved record chunk (re, im) per epilogue thread: 16 KB
 static constexpr int TILE_M = 128;           // rows of U / templates of R per tile (= UMMA M, TMEM lanes)
 static constexpr int TILE_N = 128;           // max columns (time samples) per tile
 static constexpr int BK = 64;                // K elements per TMA box = one 128-byte swizzled row of fp16
 static constexpr int TILE_BYTES = TILE_M * BK * 2;   // 16 KB
+static constexpr int RBK = 32;               // a3: K elements per TMA box (64-byte swizzled rows)
+static constexpr int RTILE_BYTES = TILE_M * RBK * 2;   // 8 KB
+static constexpr int RES_KMAX = 144;         // resident-R variant: the item's R tile (4 tiles x ceil(Kpad / 32) K blocks) <= 160 KB
+static constexpr int RMAX_STAGES = 8;        // a3 operand ring: at most 8 stages
+static constexpr int RECON_SMEM_BUDGET = 232448 - 1024 - 256;   // dynamic shared memory per CTA minus alignment and barriers
 
-struct TcReconTile { int bank, det, m0, t0, nt, slot; };   // nt consecutive time tiles starting at sample t0; partial slot
+struct TcReconTile { int bank, det, ndet, m0, t0, nt, slot; };   // detectors det..det+ndet-1 x nt consecutive time tiles from sample t0; partial slot
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
-  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 64 x 128
-  CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 64 x 128
-  CUtensorMap mapY64;                        // same array, box 64 x 64 (resident-R kernel: 64-sample tiles)
-  const __half *R16;                         // [planes][2][Mpad][Kpad]
+  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
+  CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
   int M, Mpad, Kpad, tmpl_off;
   float inv_scale;
-  int pad_[9];
+  int pad_[11];
 };
 struct TcCorrClass {
   CUtensorMap mapU;                          // [planes*Lpad rows][Npad] fp16, box 64 x 128
@@ -45,211 +51,39 @@ struct TcCorrClass {
 };
 
 // ------------------------------------------------------------------------------------------------
-// a3 + a5.  Persistent CTAs; tile = 128 templates x 128 samples of one (bank, detector); accumulators
-// re / im [128 x 128] fp32 each, double buffered in TMEM (512 columns).  Per K block of 64:
-//   re += Rre_hi Y_hi (+ Rre_hi Y_lo + Rre_lo Y_hi),  im likewise  -> 2 or 6 MMAs of 128x128x16 per K step.
+// a3 + a5.  Persistent CTAs; tile = 128 templates x 128 samples of one (bank, detector); accumulators re / im
+// [128 x 128] fp32 each, double buffered in TMEM (512 columns).  Per 16 of K: re += Rre_hi Y_hi, im += Rim_hi Y_hi (fp16)
+// and, in split mode, one fp8 MMA each carrying both hi/lo cross terms.
+// The kernel is bound by operand delivery from L2 unless R is reused (measured), so a work item is a
+// (bank, 128-template tile) with a run of (detector, time tile) pairs and, in the RES variant (split mode, Kpad <=
+// RES_KMAX), all K blocks of the item's R tile are loaded ONCE into a resident shared-memory region; only the
+// upsampled-Y blocks stream through the ring.  The streaming variant (any Kpad) moves R and Y blocks together.
 // ------------------------------------------------------------------------------------------------
-template <int PLANES>
+template <int PLANES, bool RES>
 __global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                 int n_det, int B,
-                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank) {
-  constexpr int STAGES = PLANES == 2 ? 2 : 4;
-  constexpr int STAGE_BYTES = 3 * PLANES * TILE_BYTES;        // Rre, Rim, Y per plane
+                PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank,
+                int ring_off, int n_stages) {
+  // Operand ring of K blocks of RBK = 32 (tiles of 128 rows x 32 fp16, 64-byte swizzle).  Streaming: NT = 3 * PLANES tiles
+  // per stage (Rre, Rim, Y per plane), 4 or 8 stages.  RES: 2 tiles per stage (Y fp16, Y correction), 3 stages, after the
+  // resident R region [K block][Rre, Rim, Rre corr, Rim corr].
+  constexpr int NT = RES ? 2 : 3 * PLANES;
+  constexpr int STAGE_BYTES = NT * RTILE_BYTES;
+  const int STAGES = n_stages;                                  // <= RMAX_STAGES; the resident region [0, ring_off) comes first
   extern __shared__ __align__(1024) uint8_t smem_raw[];
   uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint64_t *bars = (uint64_t *)(smem + STAGES * STAGE_BYTES);
-  uint64_t *full = bars, *empty = bars + STAGES, *tfull = bars + 2 * STAGES, *tempty = bars + 2 * STAGES + 2;
-  uint32_t *tmem_slot = (uint32_t *)(bars + 2 * STAGES + 4);
+  uint8_t *ring = smem + ring_off;
+  float4 *rec = (float4 *)(ring + STAGES * STAGE_BYTES);       // [re, im][PK_CHUNK / 4][EPI_THREADS] float4
+  uint64_t *bars = (uint64_t *)((uint8_t *)rec + REC_BYTES);
+  uint64_t *full = bars, *empty = bars + RMAX_STAGES, *tfull = bars + 2 * RMAX_STAGES, *tempty = tfull + 2, *rfull = tempty + 2, *rfree = rfull + 1;
+  uint32_t *tmem_slot = (uint32_t *)(rfree + 1);
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
     for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 8); }
-    mbar_fence_init();
-  }
-  if (warp == 1) tmem_alloc(tmem_slot, 512);
-  tc_fence_before_sync();
-  __syncthreads();
-  tc_fence_after_sync();
-  const uint32_t tmem = *tmem_slot;
-
-  if (warp == 0) {
-    // ===== TMA producer
-    if (lane == 0) {
-      int stage = 0; uint32_t phase = 0;
-      for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
-        const TcReconTile tl = tiles[ti];
-        const TcReconBank *bk = &banks[tl.bank];
-        const int nkb = (bk->Kpad + BK - 1) / BK;
-        for (int tt = 0; tt < tl.nt; ++tt)
-        for (int kb = 0; kb < nkb; ++kb) {
-          mbar_wait(&empty[stage], phase ^ 1);
-          mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
-          uint8_t *s = smem + stage * STAGE_BYTES;
-#pragma unroll
-          for (int p = 0; p < PLANES; ++p) {
-            tma_load_2d(s + (3 * p + 0) * TILE_BYTES, &bk->mapR, &full[stage], kb * BK, (p * 2 + 0) * bk->Mpad + tl.m0);
-            tma_load_2d(s + (3 * p + 1) * TILE_BYTES, &bk->mapR, &full[stage], kb * BK, (p * 2 + 1) * bk->Mpad + tl.m0);
-            tma_load_2d(s + (3 * p + 2) * TILE_BYTES, &bk->mapY, &full[stage], kb * BK, (p * n_det + tl.det) * B + tl.t0 + tt * TILE_N);
-          }
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-  } else if (warp == 1) {
-    // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers),
-    // one elected lane issues the MMAs of a K block and the commits
-    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N), idesc8 = idesc_f8_f32(TILE_M, TILE_N);
-    int stage = 0; uint32_t phase = 0; int it = 0;
-    for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
-      const TcReconTile tl = tiles[ti];
-      const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
-      for (int tt = 0; tt < tl.nt; ++tt, ++it) {
-        const int buf = it & 1;
-        mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
-        tc_fence_after_sync();
-        const uint32_t d_re = tmem + buf * 256, d_im = d_re + 128;
-        for (int kb = 0; kb < nkb; ++kb) {
-          mbar_wait(&full[stage], phase);
-          tc_fence_after_sync();
-          // one base descriptor per stage; every operand tile / K step is a constant added to its 16-byte address field
-          const uint64_t db = desc_kmajor_sw128(smem_u32(smem + stage * STAGE_BYTES));
-          const int nk = min(BK / 16, (Kpad - kb * BK) / 16);       // K is padded to 16, the last 64-wide box is zero-filled
-          if (elect_one()) {
-#pragma unroll
-            for (int k = 0; k < BK / 16; ++k) {
-              if (k >= nk) break;
-              const bool acc = (kb | k) != 0;
-              const uint64_t re_hi = db + ((0 * TILE_BYTES + k * 32) >> 4), im_hi = db + ((1 * TILE_BYTES + k * 32) >> 4),
-                             y_hi = db + ((2 * TILE_BYTES + k * 32) >> 4);
-              mma_f16_ss(d_re, re_hi, y_hi, idesc, acc);
-              mma_f16_ss(d_im, im_hi, y_hi, idesc, acc);
-              if (PLANES == 2) {
-                // the correction planes: 32 bytes = 16 of K as (e4m3, e4m3) x (e5m2, e5m2) pairs -> one fp8 MMA adds both
-                // cross terms R_hi Y_lo + R_lo Y_hi
-                const uint64_t re_8 = db + ((3 * TILE_BYTES + k * 32) >> 4), im_8 = db + ((4 * TILE_BYTES + k * 32) >> 4),
-                               y_8 = db + ((5 * TILE_BYTES + k * 32) >> 4);
-                mma_f8_ss(d_re, re_8, y_8, idesc8, true);
-                mma_f8_ss(d_im, im_8, y_8, idesc8, true);
-              }
-            }
-            mma_commit(&empty[stage]);
-            if (kb == nkb - 1) mma_commit(&tfull[buf]);
-          }
-          __syncwarp();
-          if (++stage == STAGES) { stage = 0; phase ^= 1; }
-        }
-      }
-    }
-  } else {
-    // ===== epilogue (8 warps): thread = one template (TMEM lane) x one half (64 samples) of the tile.  The running
-    // maximum is taken on the raw accumulators (the scale is a power of two, so the order is unchanged).
-    const int q = warp & 3;                       // TMEM lane quadrant this warp may access
-    const int half = (warp - 2) >> 2;             // warps 2-5: samples 0-63, warps 6-9: samples 64-127
-    int it = 0;
-    for (int ti = cta_begin[blockIdx.x]; ti < cta_begin[blockIdx.x + 1]; ++ti) {
-      const TcReconTile tl = tiles[ti];
-      const TcReconBank *bk = &banks[tl.bank];
-      const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
-      const float sc = bk->inv_scale;
-      const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < M;
-      float bp = -1.f, bre = 0.f, bim = 0.f;      // running first maximum over the unit's nt tiles (ascending time)
-      int bidx = 0;
-      for (int tt = 0; tt < tl.nt; ++tt, ++it) {
-        const int buf = it & 1;
-        const int tbase = tl.t0 + tt * TILE_N + half * (TILE_N / 2);
-        mbar_wait(&tfull[buf], (it >> 1) & 1);
-        tc_fence_after_sync();
-        const uint32_t t_re = tmem + ((uint32_t)(q * 32) << 16) + buf * 256 + half * (TILE_N / 2);
-#pragma unroll 1
-        for (int c = 0; c < TILE_N / 64; ++c) {
-          uint32_t vr[32], vi[32];
-          tmem_ld_32x32(t_re + c * 32, vr);
-          tmem_ld_32x32(t_re + 128 + c * 32, vi);
-          tmem_ld_wait();
-          const int t0c = tbase + c * 32;
-          if (t0c + 32 <= B) {
-#pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
-              const float p = fmaf(re, re, im * im);
-              if (p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
-            }
-          } else {
-#pragma unroll
-            for (int i = 0; i < 32; ++i) {
-              const float re = __uint_as_float(vr[i]), im = __uint_as_float(vi[i]);
-              const float p = fmaf(re, re, im * im);
-              if (t0c + i < B && p > bp) { bp = p; bidx = t0c + i; bre = re; bim = im; }
-            }
-          }
-          if (dbg) {
-            float *o = snr_debug + ((size_t)tl.det * 2 * M + 2 * m) * B;
-#pragma unroll
-            for (int i = 0; i < 32; ++i)
-              if (t0c + i < B) { o[t0c + i] = __uint_as_float(vr[i]) * sc; o[B + t0c + i] = __uint_as_float(vi[i]) * sc; }
-          }
-        }
-        tc_fence_before_sync();
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&tempty[buf]);
-      }
-      if (m < M) {
-        PeakPartial best;
-        best.re = bre * sc; best.im = bim * sc; best.idx = bidx;
-        best.p = (bp < 0.f) ? -1.f : best.re * best.re + best.im * best.im;
-        partial[((size_t)tl.det * Mtot + tmpl_off + m) * n_tt + tl.slot * 2 + half] = best;
-      }
-    }
-  }
-  tc_fence_before_sync();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem, 512);
-}
-
-// ------------------------------------------------------------------------------------------------
-// a3 + a5, resident-R variant (banks with Kpad <= TS_KMAX, hi + lo planes).  A work item is one (bank, 128-template tile)
-// and a run of (detector, time tile) pairs; the template tile's reconstruction rows stay ON CHIP for the whole item:
-//   R_hi (re, im) in TENSOR MEMORY as the A operand of tcgen05.mma (columns 256.., written once per item by the epilogue
-//        warps with tcgen05.st) -- 4 of the 6 MMAs of a K step then read only the Y tile from shared memory;
-//   R_lo (re, im) resident in shared memory (TMA, once per item) for the two R_lo x Y_hi MMAs.
-// Only the upsampled-Y tiles [64 samples][64 K] (hi, lo) stream through the TMA ring.  Tile = 128 templates x 64 samples,
-// re / im accumulators double buffered in TMEM columns 0..255.
-// Peak search: per 16-sample chunk the epilogue thread computes |z|^2 (packed fp32x2), the chunk maximum (3-input max),
-// and only when it beats the running maximum saves the chunk's (re, im) to a per-thread shared-memory slot; the first
-// sample attaining the maximum is located once per run from the saved chunk (same arithmetic, bit-identical p).
-// ------------------------------------------------------------------------------------------------
-static constexpr int TS_NT = 64;                        // samples per tile
-static constexpr int TS_KMAX = 256;                     // R_hi (re + im) fills TMEM columns 256..511
-static constexpr int TS_THREADS = 320;                  // warps: 0 TMA, 1 MMA, 2-9 epilogue / R loaders
-static constexpr int TS_YTILE = TS_NT * BK * 2;         // one plane of a Y stage: 8 KB
-static constexpr int TS_YSTAGE = 2 * TS_YTILE;          // hi + lo
-static constexpr int TS_CHUNK = 16;                     // samples per peak-search chunk
-static constexpr int TS_REC_BYTES = 256 * TS_CHUNK * 8; // saved record chunk per epilogue thread: 32 KB
-static constexpr int TS_MAX_YSTAGES = 8;
-
-struct TsItem { int bank, m0, det0, ndet, t0, nt, slot; };   // nt tiles of 64 samples from sample t0, for detectors det0..det0+ndet-1
-
-__global__ void __launch_bounds__(TS_THREADS, 1)
-recon_ts_kernel(const TcReconBank *__restrict__ banks, const TsItem *__restrict__ items, const int *__restrict__ cta_begin,
-                int n_det, int B, PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug,
-                int debug_bank, int rlo_bytes, int n_ys) {
-  extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
-  uint8_t *rlo = smem;                                           // [2 parts][nkb][128 rows x 64 K] fp16, 128-B swizzle
-  uint8_t *ybuf = smem + rlo_bytes;                              // [n_ys][hi, lo][64 samples x 64 K]
-  float4 *rec = (float4 *)(ybuf + n_ys * TS_YSTAGE);             // [8][256 threads] {re0, im0, re1, im1}
-  uint64_t *bars = (uint64_t *)((uint8_t *)rec + TS_REC_BYTES);
-  uint64_t *yfull = bars, *yempty = bars + TS_MAX_YSTAGES, *tfull = bars + 2 * TS_MAX_YSTAGES, *tempty = tfull + 2,
-           *rfull = tempty + 2, *rlofull = rfull + 1, *rdone = rlofull + 1;
-  uint32_t *tmem_slot = (uint32_t *)(rdone + 1);
-  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-
-  if (warp == 0 && lane == 0) {
-    for (int i = 0; i < n_ys; ++i) { mbar_init(&yfull[i], 1); mbar_init(&yempty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 8); }
-    mbar_init(rfull, 8); mbar_init(rlofull, 1); mbar_init(rdone, 1);
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], EPI_THREADS / 32); }
+    mbar_init(rfull, 1); mbar_init(rfree, 1);
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -260,178 +94,193 @@ recon_ts_kernel(const TcReconBank *__restrict__ banks, const TsItem *__restrict_
   const int i_begin = cta_begin[blockIdx.x], i_end = cta_begin[blockIdx.x + 1];
 
   if (warp == 0) {
-    // ===== TMA producer: R_lo once per item, then the Y tiles of every (detector, time tile)
+    // ===== TMA producer
     if (lane == 0) {
       int stage = 0; uint32_t phase = 0;
-      for (int ii = i_begin; ii < i_end; ++ii) {
-        const TsItem it = items[ii];
-        const TcReconBank *bk = &banks[it.bank];
-        const int nkb = (bk->Kpad + BK - 1) / BK;
-        if (ii > i_begin) mbar_wait(rdone, (uint32_t)(ii - i_begin - 1) & 1);     // previous item's MMAs have read R_lo
-        mbar_arrive_expect_tx(rlofull, 2 * nkb * TILE_BYTES);
-        for (int part = 0; part < 2; ++part)
+      for (int ti = i_begin; ti < i_end; ++ti) {
+        const TcReconTile tl = tiles[ti];
+        const TcReconBank *bk = &banks[tl.bank];
+        const int nkb = (bk->Kpad + RBK - 1) / RBK;
+        if (RES) {
+          if (ti > i_begin) mbar_wait(rfree, (uint32_t)(ti - i_begin - 1) & 1);    // the previous item's MMAs have read R
+          mbar_arrive_expect_tx(rfull, nkb * 4 * RTILE_BYTES);
           for (int kb = 0; kb < nkb; ++kb)
-            tma_load_2d(rlo + (part * nkb + kb) * TILE_BYTES, &bk->mapR, rlofull, kb * BK, (2 + part) * bk->Mpad + it.m0);
-        for (int d = 0; d < it.ndet; ++d)
-          for (int tt = 0; tt < it.nt; ++tt) {
-            const int row = (it.det0 + d) * B + it.t0 + tt * TS_NT;
-            for (int kb = 0; kb < nkb; ++kb) {
-              mbar_wait(&yempty[stage], phase ^ 1);
-              mbar_arrive_expect_tx(&yfull[stage], TS_YSTAGE);
-              uint8_t *sdst = ybuf + stage * TS_YSTAGE;
-              tma_load_2d(sdst, &bk->mapY64, &yfull[stage], kb * BK, row);
-              tma_load_2d(sdst + TS_YTILE, &bk->mapY64, &yfull[stage], kb * BK, n_det * B + row);
-              if (++stage == n_ys) { stage = 0; phase ^= 1; }
+#pragma unroll
+            for (int j = 0; j < 4; ++j) tma_load_2d(smem + (kb * 4 + j) * RTILE_BYTES, &bk->mapR, rfull, kb * RBK, j * bk->Mpad + tl.m0);
+        }
+        for (int d = 0; d < tl.ndet; ++d)
+        for (int tt = 0; tt < tl.nt; ++tt) {
+          const int yrow = (tl.det + d) * B + tl.t0 + tt * TILE_N;
+          for (int kb = 0; kb < nkb; ++kb) {
+            mbar_wait(&empty[stage], phase ^ 1);
+            mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
+            uint8_t *sdst = ring + stage * STAGE_BYTES;
+            if (RES) {
+              tma_load_2d(sdst, &bk->mapY, &full[stage], kb * RBK, yrow);
+              tma_load_2d(sdst + RTILE_BYTES, &bk->mapY, &full[stage], kb * RBK, n_det * B + yrow);
+            } else {
+#pragma unroll
+              for (int p = 0; p < PLANES; ++p) {
+                tma_load_2d(sdst + (3 * p + 0) * RTILE_BYTES, &bk->mapR, &full[stage], kb * RBK, (p * 2 + 0) * bk->Mpad + tl.m0);
+                tma_load_2d(sdst + (3 * p + 1) * RTILE_BYTES, &bk->mapR, &full[stage], kb * RBK, (p * 2 + 1) * bk->Mpad + tl.m0);
+                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, &bk->mapY, &full[stage], kb * RBK, p * n_det * B + yrow);
+              }
             }
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
+        }
       }
     }
   } else if (warp == 1) {
-    // ===== MMA issuer.  The whole warp runs the loops (uniform control flow and data: descriptors stay in uniform
-    // registers); one elected lane issues the MMAs of a K block and the commits.
-    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TS_NT), idesc8 = idesc_f8_f32(TILE_M, TS_NT);
-    int stage = 0; uint32_t phase = 0; int t_it = 0;
-    for (int ii = i_begin; ii < i_end; ++ii) {
-      const TsItem it = items[ii];
-      const int Kpad = banks[it.bank].Kpad, nkb = (Kpad + BK - 1) / BK;
-      const uint32_t ip = (uint32_t)(ii - i_begin) & 1;
-      mbar_wait(rfull, ip);
-      mbar_wait(rlofull, ip);
-      tc_fence_after_sync();
-      const uint32_t a_re0 = tmem + 256, a_im0 = a_re0 + (Kpad >> 1);
-      const uint64_t rl_re0 = desc_kmajor_sw128(smem_u32(rlo)), rl_im0 = desc_kmajor_sw128(smem_u32(rlo + nkb * TILE_BYTES));
-      const int ntile = it.ndet * it.nt;
-      for (int tl = 0; tl < ntile; ++tl, ++t_it) {
-        const int buf = t_it & 1;
-        mbar_wait(&tempty[buf], ((t_it >> 1) & 1) ^ 1);
+    // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers),
+    // one elected lane issues the MMAs of a K block and the commits
+    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N), idesc8 = idesc_f8_f32(TILE_M, TILE_N);
+    constexpr uint32_t T16 = RTILE_BYTES >> 4;                    // operand tile size in 16-byte descriptor units
+    int stage = 0; uint32_t phase = 0; int it = 0;
+    const uint64_t ring_d = desc_kmajor_sw(smem_u32(ring), RBK), res_d = desc_kmajor_sw(smem_u32(smem), RBK);
+    for (int ti = i_begin; ti < i_end; ++ti) {
+      const TcReconTile tl = tiles[ti];
+      const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + RBK - 1) / RBK;
+      if (RES) { mbar_wait(rfull, (uint32_t)(ti - i_begin) & 1); tc_fence_after_sync(); }
+      const int ntile = tl.ndet * tl.nt;
+      for (int tn = 0; tn < ntile; ++tn, ++it) {
+        const int buf = it & 1;
+        mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
-        const uint32_t d_re = tmem + buf * 128, d_im = d_re + 64;
+        const uint32_t d_re = tmem + buf * 256, d_im = d_re + 128;
         for (int kb = 0; kb < nkb; ++kb) {
-          mbar_wait(&yfull[stage], phase);
+          mbar_wait(&full[stage], phase);
           tc_fence_after_sync();
-          const uint64_t yd = desc_kmajor_sw128(smem_u32(ybuf + stage * TS_YSTAGE));
-          const int nk = min(BK / 16, (Kpad - kb * BK) / 16);
-          const uint32_t ks0 = (uint32_t)(kb * (BK / 16)) * 8;
-          const uint64_t off0 = (uint64_t)((kb * TILE_BYTES) >> 4);
+          // base descriptors; every operand tile / K step is a constant added to the 16-byte address field
+          const uint64_t sd = ring_d + (uint64_t)(stage * (STAGE_BYTES >> 4));
+          const uint64_t rd = RES ? res_d + (uint64_t)(kb * 4 * T16) : sd;
+          const bool two = Kpad - kb * RBK >= 32;                  // K is padded to 16: the last box may be half zero fill
           if (elect_one()) {
 #pragma unroll
-            for (int k = 0; k < BK / 16; ++k) {
-              if (k >= nk) break;
+            for (int k = 0; k < RBK / 16; ++k) {
+              if (k == 1 && !two) break;
               const bool acc = (kb | k) != 0;
-              const uint32_t ks = ks0 + k * 8;                                  // 16 fp16 of K = 8 TMEM columns
-              const uint64_t y_hi = yd + 2 * k, y_lo = y_hi + (TS_YTILE >> 4);
-              const uint64_t off = off0 + 2 * k;
-              mma_f16_ts(d_re, a_re0 + ks, y_hi, idesc, acc);
-              mma_f16_ts(d_im, a_im0 + ks, y_hi, idesc, acc);
-              mma_f8_ss(d_re, rl_re0 + off, y_lo, idesc8, true);                  // both cross terms in one fp8 MMA
-              mma_f8_ss(d_im, rl_im0 + off, y_lo, idesc8, true);
+              if (RES) {
+                const uint64_t y_hi = sd + 2 * k, y_8 = sd + (T16 + 2 * k);
+                mma_f16_ss(d_re, rd + (0 * T16 + 2 * k), y_hi, idesc, acc);
+                mma_f16_ss(d_im, rd + (1 * T16 + 2 * k), y_hi, idesc, acc);
+                mma_f8_ss(d_re, rd + (2 * T16 + 2 * k), y_8, idesc8, true);
+                mma_f8_ss(d_im, rd + (3 * T16 + 2 * k), y_8, idesc8, true);
+              } else {
+                const uint64_t y_hi = sd + (2 * T16 + 2 * k);
+                mma_f16_ss(d_re, sd + (0 * T16 + 2 * k), y_hi, idesc, acc);
+                mma_f16_ss(d_im, sd + (1 * T16 + 2 * k), y_hi, idesc, acc);
+                if (PLANES == 2) {
+                  // the correction planes: 32 bytes = 16 of K as (e4m3, e4m3) x (e5m2, e5m2) pairs -> one fp8 MMA adds
+                  // both cross terms R_hi Y_lo + R_lo Y_hi
+                  const uint64_t y_8 = sd + (5 * T16 + 2 * k);
+                  mma_f8_ss(d_re, sd + (3 * T16 + 2 * k), y_8, idesc8, true);
+                  mma_f8_ss(d_im, sd + (4 * T16 + 2 * k), y_8, idesc8, true);
+                }
+              }
             }
-            mma_commit(&yempty[stage]);
+            mma_commit(&empty[stage]);
             if (kb == nkb - 1) mma_commit(&tfull[buf]);
+            if (RES && kb == nkb - 1 && tn == ntile - 1) mma_commit(rfree);
           }
           __syncwarp();
-          if (++stage == n_ys) { stage = 0; phase ^= 1; }
+          if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
-      if (elect_one()) mma_commit(rdone);
-      __syncwarp();
     }
   } else {
-    // ===== epilogue warps (8): thread = template (TMEM lane) x one half (32 samples) of the tile; they also place R_hi of
-    // each item in tensor memory (warps 2-5: real rows, 6-9: imaginary rows)
-    const int q = warp & 3, half = (warp - 2) >> 2, etid = threadIdx.x - 64;
+    // ===== epilogue (16 warps, four per scheduler): thread = one template (TMEM lane) x one 32-sample slice of the tile.
+    // Peak search (first maximum of |z|^2): per 8-sample chunk the thread computes |z|^2 with packed
+    // fp32x2 arithmetic and the chunk maximum (3-input max); only when that beats the running maximum (strict >, so an
+    // earlier chunk keeps a tie) it saves the chunk's (re, im) to its shared-memory slot.  The first sample attaining the
+    // maximum is located once per run from the saved chunk with the same arithmetic (bit-identical p).  The raw
+    // accumulators are compared: the operand scale is a power of two, so the order is unchanged.
+    const int q = warp & 3, cs = (warp - 2) >> 2, etid = threadIdx.x - 64;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-    int t_it = 0;
-    for (int ii = i_begin; ii < i_end; ++ii) {
-      const TsItem it = items[ii];
-      const TcReconBank *bk = &banks[it.bank];
-      const int M = bk->M, Kpad = bk->Kpad, tmpl_off = bk->tmpl_off;
-      const int m = it.m0 + q * 32 + lane;
+    float4 *rec_re = rec + etid, *rec_im = rec + (PK_CHUNK / 4) * EPI_THREADS + etid;   // conflict-free 16-byte slots
+    int it = 0;
+    for (int ti = i_begin; ti < i_end; ++ti) {
+      const TcReconTile tl = tiles[ti];
+      const TcReconBank *bk = &banks[tl.bank];
+      const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
       const float sc = bk->inv_scale;
-      {
-        // every MMA of the previous item has completed (this warp waited for tfull of its last tile): R_hi may be replaced
-        const uint4 *src = reinterpret_cast<const uint4 *>(bk->R16 + ((size_t)half * bk->Mpad + m) * Kpad);
-        const uint32_t tdst = tmem + lane_base + 256 + half * (Kpad >> 1);
-        const int n16 = Kpad >> 4;
-#pragma unroll 4
-        for (int c = 0; c < n16; ++c) {
-          const uint4 a = __ldg(src + 2 * c), b = __ldg(src + 2 * c + 1);
-          const uint32_t v[8] = {a.x, a.y, a.z, a.w, b.x, b.y, b.z, b.w};
-          tmem_st_32x8(tdst + c * 8, v);
-        }
-        tmem_st_wait();
-        tc_fence_before_sync();
+      const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < M;
+      for (int d = 0; d < tl.ndet; ++d) {
+      const int det = tl.det + d;
+      float bp = -1.f;                               // running first maximum over the run's nt tiles (ascending time)
+      int bt0 = 0;
+      for (int tt = 0; tt < tl.nt; ++tt, ++it) {
+        const int buf = it & 1;
+        const int tbase = tl.t0 + tt * TILE_N + cs * 32;
+        mbar_wait(&tfull[buf], (it >> 1) & 1);
+        tc_fence_after_sync();
+        const uint32_t t_re = tmem + lane_base + buf * 256 + cs * 32;
+        uint32_t vr[32], vi[32];
+        tmem_ld_32x32(t_re, vr);
+        tmem_ld_32x32(t_re + 128, vi);
+        tmem_ld_wait();
+        tc_fence_before_sync();                        // this warp's part of the accumulators is in registers: release the buffer
         __syncwarp();
-        if (lane == 0) mbar_arrive(rfull);
-      }
-      const bool dbg = snr_debug != nullptr && it.bank == debug_bank && m < M;
-      for (int d = 0; d < it.ndet; ++d) {
-        const int det = it.det0 + d;
-        float bp = -1.f;
-        int bt0 = 0;
-        for (int tt = 0; tt < it.nt; ++tt, ++t_it) {
-          const int buf = t_it & 1;
-          const int tbase = it.t0 + tt * TS_NT + half * 32;
-          mbar_wait(&tfull[buf], (t_it >> 1) & 1);
-          tc_fence_after_sync();
-          const uint32_t t_re = tmem + lane_base + buf * 128 + half * 32;
-          uint32_t vr[32], vi[32];
-          tmem_ld_32x32(t_re, vr);
-          tmem_ld_32x32(t_re + 64, vi);
-          tmem_ld_wait();
-          tc_fence_before_sync();
-          __syncwarp();
-          if (lane == 0) mbar_arrive(&tempty[buf]);                 // the accumulators are in registers: release the buffer
+        if (lane == 0) mbar_arrive(&tempty[buf]);
+        // chunk maxima are independent; the running-maximum chain is one compare + select per chunk and the record
+        // stores are predicated (no vote / branch on the chain).  Only a buffer's last tile can be ragged: that case is
+        // a separate copy of the loop, chosen once per tile.
+        auto scan = [&](auto ragged_tag) {
+          constexpr bool RAGGED = decltype(ragged_tag)::value;
 #pragma unroll
-          for (int c = 0; c < 32 / TS_CHUNK; ++c) {
-            const int t0c = tbase + c * TS_CHUNK;
-            float p[TS_CHUNK];
+          for (int c = 0; c < 32 / PK_CHUNK; ++c) {
+            const int t0c = tbase + c * PK_CHUNK;
+            float p[PK_CHUNK];
 #pragma unroll
-            for (int i = 0; i < TS_CHUNK; i += 2)
-              abs2_x2(__uint_as_float(vr[c * TS_CHUNK + i]), __uint_as_float(vr[c * TS_CHUNK + i + 1]),
-                      __uint_as_float(vi[c * TS_CHUNK + i]), __uint_as_float(vi[c * TS_CHUNK + i + 1]), p[i], p[i + 1]);
-            if (t0c + TS_CHUNK > B) {
+            for (int i = 0; i < PK_CHUNK; i += 2)
+              abs2_x2(__uint_as_float(vr[c * PK_CHUNK + i]), __uint_as_float(vr[c * PK_CHUNK + i + 1]),
+                      __uint_as_float(vi[c * PK_CHUNK + i]), __uint_as_float(vi[c * PK_CHUNK + i + 1]), p[i], p[i + 1]);
+            if (RAGGED) {
 #pragma unroll
-              for (int i = 0; i < TS_CHUNK; ++i) if (t0c + i >= B) p[i] = -1.f;
+              for (int i = 0; i < PK_CHUNK; ++i) if (t0c + i >= B) p[i] = -1.f;
             }
             float cm = p[0];
 #pragma unroll
-            for (int i = 1; i + 1 < TS_CHUNK; i += 2) cm = fmaxf(cm, fmaxf(p[i], p[i + 1]));
-            cm = fmaxf(cm, p[TS_CHUNK - 1]);
-            const bool rec_now = cm > bp;                          // strict: an earlier chunk keeps a tie (first maximum)
-            if (__any_sync(0xffffffffu, rec_now)) {
-              if (rec_now) {
-                bp = cm; bt0 = t0c;
+            for (int i = 1; i + 1 < PK_CHUNK; i += 2) cm = fmaxf(cm, fmaxf(p[i], p[i + 1]));
+            cm = fmaxf(cm, p[PK_CHUNK - 1]);
+            if (cm > bp) {                             // strict: an earlier chunk keeps a tie (first maximum)
+              bp = cm; bt0 = t0c;
 #pragma unroll
-                for (int j = 0; j < TS_CHUNK / 2; ++j)
-                  rec[j * 256 + etid] = make_float4(__uint_as_float(vr[c * TS_CHUNK + 2 * j]), __uint_as_float(vi[c * TS_CHUNK + 2 * j]),
-                                                    __uint_as_float(vr[c * TS_CHUNK + 2 * j + 1]), __uint_as_float(vi[c * TS_CHUNK + 2 * j + 1]));
+              for (int j = 0; j < PK_CHUNK / 4; ++j) {  // the loaded registers are consecutive: plain 16-byte stores
+                const int o = c * PK_CHUNK + 4 * j;
+                rec_re[j * EPI_THREADS] = make_float4(__uint_as_float(vr[o]), __uint_as_float(vr[o + 1]), __uint_as_float(vr[o + 2]), __uint_as_float(vr[o + 3]));
+                rec_im[j * EPI_THREADS] = make_float4(__uint_as_float(vi[o]), __uint_as_float(vi[o + 1]), __uint_as_float(vi[o + 2]), __uint_as_float(vi[o + 3]));
               }
             }
           }
-          if (dbg) {
-            float *o = snr_debug + ((size_t)det * 2 * M + 2 * m) * B;
+        };
+        if (tl.t0 + tt * TILE_N + TILE_N > B) scan(std::true_type()); else scan(std::false_type());
+        if (dbg) {
+          float *o = snr_debug + ((size_t)det * 2 * M + 2 * m) * B;
 #pragma unroll
-            for (int i = 0; i < 32; ++i)
-              if (tbase + i < B) { o[tbase + i] = __uint_as_float(vr[i]) * sc; o[B + tbase + i] = __uint_as_float(vi[i]) * sc; }
-          }
+          for (int i = 0; i < 32; ++i)
+            if (tbase + i < B) { o[tbase + i] = __uint_as_float(vr[i]) * sc; o[B + tbase + i] = __uint_as_float(vi[i]) * sc; }
         }
-        if (m < M) {
-          PeakPartial best;
-          best.p = -1.f; best.idx = 0; best.re = 0.f; best.im = 0.f;
-          if (bp >= 0.f) {
-            bool found = false;
+      }
+      if (m < M) {
+        PeakPartial best;
+        best.p = -1.f; best.idx = 0; best.re = 0.f; best.im = 0.f;
+        if (bp >= 0.f) {
+          bool found = false;
 #pragma unroll
-            for (int j = 0; j < TS_CHUNK / 2; ++j) {
-              const float4 v = rec[j * 256 + etid];
-              const float p0 = __fmaf_rn(v.y, v.y, __fmul_rn(v.x, v.x)), p1 = __fmaf_rn(v.w, v.w, __fmul_rn(v.z, v.z));
-              if (!found && p0 == bp) { found = true; best.idx = bt0 + 2 * j; best.re = v.x * sc; best.im = v.y * sc; }
-              if (!found && p1 == bp) { found = true; best.idx = bt0 + 2 * j + 1; best.re = v.z * sc; best.im = v.w * sc; }
+          for (int j = 0; j < PK_CHUNK / 4; ++j) {
+            const float4 a = rec_re[j * EPI_THREADS], b = rec_im[j * EPI_THREADS];
+            const float re4[4] = {a.x, a.y, a.z, a.w}, im4[4] = {b.x, b.y, b.z, b.w};
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+              const float pp = __fmaf_rn(im4[i], im4[i], __fmul_rn(re4[i], re4[i]));
+              if (!found && pp == bp) { found = true; best.idx = bt0 + 4 * j + i; best.re = re4[i] * sc; best.im = im4[i] * sc; }
             }
-            best.p = best.re * best.re + best.im * best.im;
           }
-          partial[((size_t)det * Mtot + tmpl_off + m) * n_tt + it.slot * 2 + half] = best;
+          best.p = best.re * best.re + best.im * best.im;
         }
+        partial[((size_t)det * Mtot + tmpl_off + m) * n_tt + tl.slot * 4 + cs] = best;
+      }
       }
     }
   }
@@ -709,7 +558,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 struct TcPlan {
   int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
-  TsItem *ts_items_dev; int *ts_begin_dev; int n_ts_items, ts_grid, ts_smem, ts_rlo_bytes, ts_ystages;   // resident-R a3
+  TcReconTile *res_items_dev; int *res_begin_dev; int n_res_items, res_grid, res_ring_off, res_stages, str_stages;   // resident-R a3
   int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
@@ -725,9 +574,9 @@ static int recon_run_tiles(int B, long long n_mtile_units) {
   while (nt * 2 <= ntile && n_mtile_units * ((ntile + 2 * nt - 1) / (2 * nt)) >= 3 * 148) nt *= 2;
   return nt;
 }
-int tc_time_splits(int B, long long n_mtile_units) {          // partial peaks per template: 2 halves per run
+int tc_time_splits(int B, long long n_mtile_units) {          // partial peaks per template: 4 column slices per run
   const int ntile = (B + TILE_N - 1) / TILE_N, nt = recon_run_tiles(B, n_mtile_units);
-  return 2 * ((ntile + nt - 1) / nt);
+  return 4 * ((ntile + nt - 1) / nt);
 }
 
 // Longest-processing-time assignment of work items to `grid` persistent CTAs: items sorted by decreasing cost, each given
@@ -775,16 +624,17 @@ static EncodeTiledFn get_encode() {
   return fn;
 }
 
-// fp16 row-major [rows][cols] (cols % 64 == 0), box = 64 columns x 128 rows, 128-byte swizzle
-static bool make_map(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, int box_rows) {
+// fp16 row-major [rows][cols], box = box_cols (64 / 32 / 16) columns x box_rows rows, swizzle = the box's row width (128 / 64 / 32 B)
+static bool make_map(CUtensorMap *m, const void *base, uint64_t rows, uint64_t cols, int box_rows, int box_cols) {
   EncodeTiledFn enc = get_encode();
   if (!enc) { set_error("stream_create: cuTensorMapEncodeTiled is not available from the driver"); return false; }
   cuuint64_t dims[2] = {cols, rows};
   cuuint64_t strides[1] = {cols * 2};
-  cuuint32_t box[2] = {BK, (cuuint32_t)box_rows};
+  cuuint32_t box[2] = {(cuuint32_t)box_cols, (cuuint32_t)box_rows};
+  const CUtensorMapSwizzle sw = box_cols == 16 ? CU_TENSOR_MAP_SWIZZLE_32B : (box_cols == 32 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_128B);
   cuuint32_t estr[2] = {1, 1};
   CUresult r = enc(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
-                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, sw, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
                    CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
   if (r != CUDA_SUCCESS) { set_error("stream_create: cuTensorMapEncodeTiled failed (%d) for [%llu][%llu]", (int)r,
                                      (unsigned long long)rows, (unsigned long long)cols); return false; }
@@ -822,7 +672,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   for (size_t ci = 0; ci < classes.size(); ++ci) {
     const CorrClass &c = classes[ci];
     memset(&cm[ci], 0, sizeof(TcCorrClass));
-    if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad, TILE_M)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    if (!make_map(&cm[ci].mapU, c.U16, (uint64_t)planes * c.Lpad, (uint64_t)c.Npad, TILE_M, BK)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     const int nseg = tc_k_segments(c.Npad);
     const int kseg = ((c.Npad + nseg - 1) / nseg + BK - 1) / BK * BK;
     struct Sub { int det, c0, w; };
@@ -856,95 +706,80 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
       }
   }
   p->n_cunits = (int)cu.size();
-  // ---- a3: tensor maps per bank.  Banks whose concatenated basis axis fits the resident-R kernel (split mode, Kpad <=
-  //      TS_KMAX) become TsItems; the others are tiled (bank, template tile, detector, time tile) for the streaming kernel
+  // ---- a3: two tensor maps per bank.  Banks whose R tile fits the resident region (split mode, Kpad <= RES_KMAX) become
+  //      items (bank, template tile, detector group, run of time tiles) of the resident-R kernel; the others are tiled
+  //      (bank, template tile, detector, run of time tiles) for the streaming kernel
   std::vector<TcReconBank> rb(banks.size());
-  std::vector<TcReconTile> rt;
-  std::vector<TsItem> ts;
-  std::vector<char> is_ts(banks.size(), 0);
-  for (size_t b = 0; b < banks.size(); ++b) {
-    const ReconBank &k = banks[b];
-    memset(&rb[b], 0, sizeof(TcReconBank));
-    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M) ||
-        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M) ||
-        !make_map(&rb[b].mapY64, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TS_NT)) { tc_plan_destroy(p); return LLOID_ECUDA; }
-    rb[b].R16 = k.R16;
-    rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
-    is_ts[b] = (planes == 2 && k.Kpad <= TS_KMAX && !getenv("LLOID_DEBUG_NO_TS")) ? 1 : 0;
-  }
+  std::vector<TcReconTile> rt, ri;
+  std::vector<char> is_res(banks.size(), 0);
   int dev = 0, sms = 148;
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   long long n_mu = 0, n_bm = 0;
-  int nkb_max = 1;
+  int res_kmax = 0;
   for (size_t b = 0; b < banks.size(); ++b) {
-    const long long mt = (banks[b].M + TILE_M - 1) / TILE_M;
-    if (is_ts[b]) { n_bm += mt; nkb_max = std::max(nkb_max, (banks[b].Kpad + BK - 1) / BK); }
+    const ReconBank &k = banks[b];
+    memset(&rb[b], 0, sizeof(TcReconBank));
+    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK) ||
+        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
+    is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && !getenv("LLOID_DEBUG_NO_RES")) ? 1 : 0;
+    const long long mt = (k.M + TILE_M - 1) / TILE_M;
+    if (is_res[b]) { n_bm += mt; res_kmax = std::max(res_kmax, k.Kpad); }
     else n_mu += mt * n_det;
   }
   const int nt = recon_run_tiles(B, n_mu), ntile = (B + TILE_N - 1) / TILE_N;
-  p->n_tt = n_mu ? tc_time_splits(B, n_mu) : 2;
-  // resident-R items: one (bank, template tile) per item; split by detector, then by runs of time tiles, until the
-  // persistent grid has a few items per SM
-  const int tiles64 = (B + TS_NT - 1) / TS_NT;
+  p->n_tt = n_mu ? tc_time_splits(B, n_mu) : 4;
+  // resident items: split by detector, then into runs of time tiles, until the persistent grid has a few items per SM
   const int det_split = (n_bm < 4LL * sms && n_det > 1) ? n_det : 1;
   int r_time = 1;
-  while (n_bm * det_split * r_time < 2LL * sms && tiles64 / (r_time * 2) >= 2) r_time *= 2;
-  const int nt_run = (tiles64 + r_time - 1) / r_time, n_runs = (tiles64 + nt_run - 1) / nt_run;
-  if (n_bm) p->n_tt = std::max(p->n_tt, 2 * n_runs);
+  while (n_bm * det_split * r_time < 2LL * sms && ntile / (r_time * 2) >= 2) r_time *= 2;
+  const int nt_run = (ntile + r_time - 1) / r_time, n_runs = (ntile + nt_run - 1) / nt_run;
+  if (n_bm) p->n_tt = std::max(p->n_tt, 4 * n_runs);
   for (size_t b = 0; b < banks.size(); ++b) {
     const ReconBank &k = banks[b];
     for (int m0 = 0; m0 < k.M; m0 += TILE_M) {
-      if (is_ts[b]) {
+      if (is_res[b]) {
         const int nd = n_det / det_split;
         for (int dg = 0; dg < det_split; ++dg)
           for (int r = 0; r < n_runs; ++r)
-            ts.push_back({(int)b, m0, dg * nd, nd, r * nt_run * TS_NT, std::min(nt_run, tiles64 - r * nt_run), r});
+            ri.push_back({(int)b, dg * nd, nd, m0, r * nt_run * TILE_N, std::min(nt_run, ntile - r * nt_run), r});
       } else {
         for (int det = 0; det < n_det; ++det)
-          for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
+          for (int i0 = 0; i0 < ntile; i0 += nt) rt.push_back({(int)b, det, 1, m0, i0 * TILE_N, std::min(nt, ntile - i0), i0 / nt});
       }
     }
   }
-  p->n_ts_items = (int)ts.size();
-  p->ts_grid = std::max(1, std::min(p->n_ts_items, sms));
-  p->ts_rlo_bytes = 2 * nkb_max * TILE_BYTES;
-  p->ts_ystages = std::min(TS_MAX_YSTAGES, (232448 - 1024 - 256 - p->ts_rlo_bytes - TS_REC_BYTES) / TS_YSTAGE);
-  p->ts_smem = 1024 + p->ts_rlo_bytes + p->ts_ystages * TS_YSTAGE + TS_REC_BYTES + 256;
+  p->n_res_items = (int)ri.size();
+  p->res_grid = std::max(1, std::min(p->n_res_items, sms));
+  p->res_ring_off = ((res_kmax + RBK - 1) / RBK) * 4 * RTILE_BYTES;
+  p->res_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off) / (2 * RTILE_BYTES));
+  p->str_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES) / (3 * planes * RTILE_BYTES));
   p->n_rtiles = (int)rt.size();
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
   std::vector<int> cbegin, rbegin;
   lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1] + u.nt[2] + u.nt[3]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
-  lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * ((rb[t.bank].Kpad + BK - 1) / BK + 1); }, rbegin);
-  std::vector<int> tsbegin;
-  // cost in cycles: per tile the larger of the MMA stream (6 MMAs of 32 cycles per 16 of K) and the peak-search epilogue,
-  // plus the once-per-item load of the template tile's R
-  lpt_assign(ts, p->ts_grid, [&](const TsItem &t) {
+  lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, rbegin);
+  std::vector<int> ibegin;
+  // cost in cycles: 4 MMAs of ~97 cycles per 16 of K per tile (at least the epilogue's ~600), plus the once-per-item R load
+  lpt_assign(ri, p->res_grid, [&](const TcReconTile &t) {
     const long long kp = rb[t.bank].Kpad;
-    return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 192, 450) + kp * 16 + 1500; }, tsbegin);
-  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->ts_items_dev, ts) ||
-      !plan_upload(p, &p->ts_begin_dev, tsbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+    return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 388, 600) + 3000 + kp * 8; }, ibegin);
+  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->res_items_dev, ri) ||
+      !plan_upload(p, &p->res_begin_dev, ibegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
-  const int rstages = planes == 2 ? 2 : 4;
-  p->recon_smem = rstages * 3 * planes * TILE_BYTES + 1024 + 256;
+  p->recon_smem = RECON_SMEM_BUDGET + 1024 + 256;
   p->corr_smem = (planes == 2 ? 4 : 6) * planes * TILE_BYTES + 2 * planes * STRIP_PLANE + XWIN_TOTAL * 4 + 1024 + 256;
   cudaError_t e;
   if (planes == 2) {
-    e = cudaFuncSetAttribute(recon_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
+    e = cudaFuncSetAttribute(recon_tc_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(recon_tc_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(corr_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->corr_smem);
   } else {
-    e = cudaFuncSetAttribute(recon_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
+    e = cudaFuncSetAttribute(recon_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(corr_tc_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->corr_smem);
-  }
-  if (e == cudaSuccess && p->n_ts_items) {
-    if (p->ts_ystages < 2) { set_error("stream_create: no shared memory left for the Y stages of the resident-R kernel"); tc_plan_destroy(p); return LLOID_EINVAL; }
-    // the limit is per function and device, not per stream: always opt in to the device maximum so that streams with
-    // different resident-R footprints can coexist in one process
-    int optin = 0;
-    cudaDeviceGetAttribute(&optin, cudaDevAttrMaxSharedMemoryPerBlockOptin, dev);
-    e = cudaFuncSetAttribute(recon_ts_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, std::max(optin, p->ts_smem));
   }
   if (e != cudaSuccess) { set_error("stream_create: cudaFuncSetAttribute: %s", cudaGetErrorString(e)); tc_plan_destroy(p); return LLOID_ECUDA; }
   *out = p;
@@ -961,30 +796,22 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
 }
 
 int tc_plan_n_tt(const TcPlan *p) { return p->n_tt; }
-int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_ts_items ? 1 : 0); }
+int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_res_items ? 1 : 0); }
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
-  if (p->n_ts_items)
-    recon_ts_kernel<<<p->ts_grid, TS_THREADS, p->ts_smem, st>>>(p->rbanks_dev, p->ts_items_dev, p->ts_begin_dev, p->n_det, p->B, partial, Mtot,
-                                                              p->n_tt, snr_debug, debug_bank, p->ts_rlo_bytes, p->ts_ystages);
-  {
+  if (p->n_res_items) {
+    recon_tc_kernel<2, true><<<p->res_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->res_items_dev, p->res_begin_dev, p->n_det, p->B,
+                                                                              partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off, p->res_stages);
     cudaError_t e0 = cudaGetLastError();
-    if (e0 != cudaSuccess || p->n_rtiles == 0) {
-      if (e0 != cudaSuccess) {
-        cudaFuncAttributes fa; memset(&fa, 0, sizeof(fa));
-        cudaFuncGetAttributes(&fa, recon_ts_kernel);
-        int dev = -1; cudaGetDevice(&dev);
-        fprintf(stderr, "lloid: recon_ts_kernel launch failed: grid %d smem %d rlo %d ystages %d items %d: %s; func maxDyn %d static %zu regs %d dev %d\n", p->ts_grid, p->ts_smem, p->ts_rlo_bytes, p->ts_ystages, p->n_ts_items, cudaGetErrorString(e0), fa.maxDynamicSharedSizeBytes, fa.sharedSizeBytes, fa.numRegs, dev);
-      }
-      return e0;
-    }
+    if (e0 != cudaSuccess) return e0;
   }
+  if (p->n_rtiles == 0) return cudaSuccess;
   if (p->planes == 2)
-    recon_tc_kernel<2><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
+    recon_tc_kernel<2, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
+                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages);
   else
-    recon_tc_kernel<1><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank);
+    recon_tc_kernel<1, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
+                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages);
   return cudaGetLastError();
 }
 

@@ -107,6 +107,12 @@ __device__ __forceinline__ uint64_t desc_kmajor_sw128(uint32_t smem_addr) {
   return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)1 << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
          ((uint64_t)2 << 61);
 }
+// The same for a box of w = 64 / 32 / 16 fp16 columns written with the 128- / 64- / 32-byte swizzle: rows of 2 w bytes,
+// 8-row groups 16 w bytes apart (SBO), layout type 2 / 4 / 6 in bits 61-63; K advances by +32 B inside the row.
+__device__ __forceinline__ uint64_t desc_kmajor_sw(uint32_t smem_addr, int w) {
+  const uint64_t sbo = (uint64_t)(16 * w) >> 4, layout = w == 64 ? 2 : (w == 32 ? 4 : 6);
+  return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)1 << 16) | (sbo << 32) | ((uint64_t)1 << 46) | (layout << 61);
+}
 // K-major operand without swizzle ("interleave"): core matrix = 8 rows x 16 B contiguous (128 B); LBO = byte stride
 // between the two core matrices along K of one MMA (K = 16 fp16), SBO = byte stride between 8-row groups.
 __device__ __forceinline__ uint64_t desc_kmajor_nosw(uint32_t smem_addr, uint32_t lbo_bytes, uint32_t sbo_bytes) {
