@@ -31,20 +31,22 @@ static constexpr int TILE_M = 128;           // rows of U / templates of R per t
 static constexpr int TILE_N = 128;           // max columns (time samples) per tile
 static constexpr int BK = 64;                // K elements per TMA box = one 128-byte swizzled row of fp16
 static constexpr int TILE_BYTES = TILE_M * BK * 2;   // 16 KB
-static constexpr int RBK = 32;               // a3: K elements per TMA box (64-byte swizzled rows)
-static constexpr int RTILE_BYTES = TILE_M * RBK * 2;   // 8 KB
+static constexpr int RBK_RES = 32;           // a3 resident variant: K elements per TMA box (64-byte swizzled rows)
+static constexpr int RBK_STR = 64;           // a3 streaming variant: 128-byte swizzled rows (fewer barrier round trips per K)
 static constexpr int RES_KMAX = 144;         // resident-R variant: the item's R tile (4 tiles x ceil(Kpad / 32) K blocks) <= 160 KB
 static constexpr int RMAX_STAGES = 8;        // a3 operand ring: at most 8 stages
 static constexpr int RECON_SMEM_BUDGET = 232448 - 1024 - 256;   // dynamic shared memory per CTA minus alignment and barriers
 
 struct TcReconTile { int bank, det, ndet, m0, t0, nt, slot; };   // detectors det..det+ndet-1 x nt consecutive time tiles from sample t0; partial slot
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
-  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
+  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle (resident variant)
   CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
+  CUtensorMap mapR64, mapY64;                // the same arrays, box 64 x 128, 128-byte swizzle (streaming variant)
   int M, Mpad, Kpad, tmpl_off;
   float inv_scale;
   int pad_[11];
 };
+static_assert(sizeof(TcReconBank) % 64 == 0, "CUtensorMap members need 64-byte alignment");
 struct TcCorrClass {
   CUtensorMap mapU;                          // [planes*Lpad rows][Npad] fp16, box 64 x 128
   int pad_[32];
@@ -65,7 +67,9 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
                 int n_det, int B,
                 PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank,
                 int ring_off, int n_stages) {
-  // Operand ring of K blocks of RBK = 32 (tiles of 128 rows x 32 fp16, 64-byte swizzle).  Streaming: NT = 3 * PLANES tiles
+  constexpr int RBK = RES ? RBK_RES : RBK_STR;
+  constexpr int RTILE_BYTES = TILE_M * RBK * 2;
+  // Operand ring of K blocks of RBK (tiles of 128 rows x RBK fp16).  Streaming: NT = 3 * PLANES tiles
   // per stage (Rre, Rim, Y per plane), 4 or 8 stages.  RES: 2 tiles per stage (Y fp16, Y correction), 3 stages, after the
   // resident R region [K block][Rre, Rim, Rre corr, Rim corr].
   constexpr int NT = RES ? 2 : 3 * PLANES;
@@ -121,9 +125,9 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
             } else {
 #pragma unroll
               for (int p = 0; p < PLANES; ++p) {
-                tma_load_2d(sdst + (3 * p + 0) * RTILE_BYTES, &bk->mapR, &full[stage], kb * RBK, (p * 2 + 0) * bk->Mpad + tl.m0);
-                tma_load_2d(sdst + (3 * p + 1) * RTILE_BYTES, &bk->mapR, &full[stage], kb * RBK, (p * 2 + 1) * bk->Mpad + tl.m0);
-                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, &bk->mapY, &full[stage], kb * RBK, p * n_det * B + yrow);
+                tma_load_2d(sdst + (3 * p + 0) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 0) * bk->Mpad + tl.m0);
+                tma_load_2d(sdst + (3 * p + 1) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 1) * bk->Mpad + tl.m0);
+                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, &bk->mapY64, &full[stage], kb * RBK, p * n_det * B + yrow);
               }
             }
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -154,11 +158,11 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           // base descriptors; every operand tile / K step is a constant added to the 16-byte address field
           const uint64_t sd = ring_d + (uint64_t)(stage * (STAGE_BYTES >> 4));
           const uint64_t rd = RES ? res_d + (uint64_t)(kb * 4 * T16) : sd;
-          const bool two = Kpad - kb * RBK >= 32;                  // K is padded to 16: the last box may be half zero fill
+          const int nk = min(RBK / 16, (Kpad - kb * RBK) / 16);    // K is padded to 16: the last box may be partly zero fill
           if (elect_one()) {
 #pragma unroll
             for (int k = 0; k < RBK / 16; ++k) {
-              if (k == 1 && !two) break;
+              if (k >= nk) break;
               const bool acc = (kb | k) != 0;
               if (RES) {
                 const uint64_t y_hi = sd + 2 * k, y_8 = sd + (T16 + 2 * k);
@@ -720,10 +724,13 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   for (size_t b = 0; b < banks.size(); ++b) {
     const ReconBank &k = banks[b];
     memset(&rb[b], 0, sizeof(TcReconBank));
-    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK) ||
-        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_RES) ||
+        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK_RES) ||
+        !make_map(&rb[b].mapR64, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_STR) ||
+        !make_map(&rb[b].mapY64, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
-    is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && !getenv("LLOID_DEBUG_NO_RES")) ? 1 : 0;
+    // resident R pays when the item reuses it over enough tiles (short buffers, config 4, stream R with Y instead)
+    is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && (long long)n_det * ((B + TILE_N - 1) / TILE_N) >= 8) ? 1 : 0;
     const long long mt = (k.M + TILE_M - 1) / TILE_M;
     if (is_res[b]) { n_bm += mt; res_kmax = std::max(res_kmax, k.Kpad); }
     else n_mu += mt * n_det;
@@ -752,9 +759,9 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   }
   p->n_res_items = (int)ri.size();
   p->res_grid = std::max(1, std::min(p->n_res_items, sms));
-  p->res_ring_off = ((res_kmax + RBK - 1) / RBK) * 4 * RTILE_BYTES;
-  p->res_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off) / (2 * RTILE_BYTES));
-  p->str_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES) / (3 * planes * RTILE_BYTES));
+  p->res_ring_off = ((res_kmax + RBK_RES - 1) / RBK_RES) * 4 * TILE_M * RBK_RES * 2;
+  p->res_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off) / (2 * TILE_M * RBK_RES * 2));
+  p->str_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES) / (3 * planes * TILE_M * RBK_STR * 2));
   p->n_rtiles = (int)rt.size();
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
