@@ -59,7 +59,9 @@ typedef struct {
 /* Per-template, per-buffer trigger (time, SNR, phase; integer sample). */
 typedef struct {
   float snr;           /* max_k |rho_2j[k] + i rho_2j+1[k]| over the pushed buffer                            */
-  int32_t sample;      /* first k in [0, buffer_len) attaining it (-1 if below options.threshold)            */
+  int32_t sample;      /* first k of the trigger window attaining it: in [0, buffer_len), or in [-trigger_overlap, 0)
+                          when the peak lies in the overlap with the previous buffer; LLOID_NO_TRIGGER if snr is
+                          below options.threshold                                                              */
   float phase;         /* atan2(rho_2j+1[k], rho_2j[k]) at that k                                             */
 } lloid_peak;
 
@@ -68,7 +70,21 @@ typedef struct {
   int32_t n_up;        /* upsampler half length in input samples; default 8 (only 8 supported) */
   int32_t precision;   /* lloid_precision; default LLOID_PREC_F16_SPLIT                                      */
   float threshold;     /* report only peaks with snr >= threshold; 0 = report every template's peak          */
+  int32_t trigger_overlap; /* samples by which the trigger window of a push extends back into the previous buffer
+                          (Fig. 5: light travel time + 0.005 s, e.g. 67 at 2048 Hz); default 0.
+                          0 <= trigger_overlap < buffer_len; needs a tensor-core precision                       */
 } lloid_options;
+#define LLOID_NO_TRIGGER (-2147483647 - 1)
+
+/* One coincident event of a bank in one trigger window. */
+#define LLOID_MAX_DET 4
+typedef struct {
+  int32_t template_index; /* template (index in the stream's peak order) of the event, -1 = no coincidence in this bank */
+  int32_t det_mask;       /* bit a set: detector a takes part                                                     */
+  float net_snr;          /* sqrt(sum over participating detectors of snr^2)                                       */
+  int32_t reserved;
+  float snr[LLOID_MAX_DET]; int32_t sample[LLOID_MAX_DET]; float phase[LLOID_MAX_DET]; /* the participating triggers */
+} lloid_event;
 
 typedef struct lloid_bank lloid_bank;      /* opaque, immutable after create; owns host+device copies of U, R */
 typedef struct lloid_stream lloid_stream;  /* opaque; owns the device rings / state of (banks x detectors)    */
@@ -100,6 +116,17 @@ void lloid_stream_destroy(lloid_stream *stream);
  * Buffers are caller-owned and must stay valid until the stream reaches the end of this push. */
 int lloid_stream_push(lloid_stream *stream, const float *strain, lloid_peak *peaks, float *snr_debug,
                       int32_t debug_bank);
+
+/* Coincidence formation and clustering on the triggers of one push, asynchronous on the stream's
+ * cuda_stream.  A trigger exists where peaks[det][j].sample != LLOID_NO_TRIGGER.  For every template the detector set
+ * (>= 2 detectors of the SAME template, every pair within its window) with the largest network SNR is its candidate;
+ * each bank keeps the candidate with the highest network SNR (ties: lower bit mask, lower template index).
+ *   peaks       DEVICE, [n_detectors][sum_b M_b] as written by lloid_stream_push (n_detectors <= LLOID_MAX_DET)
+ *   dt_samples  HOST, [n_detectors][n_detectors] symmetric coincidence windows in strain samples, inclusive
+ *               (light travel time + 0.005 s; e.g. ceil(0.0150 * f0) for H-L)
+ *   events      DEVICE, [n_banks] lloid_event
+ * Errors: EINVAL (null pointer, more than LLOID_MAX_DET detectors, negative window), ECUDA. */
+int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int32_t *dt_samples, lloid_event *events);
 
 /* Same through HOST buffers: copies strain host->device, pushes, copies peaks device->host and waits for
  * the stream.  strain_host [n_detectors][buffer_len], peaks_host [n_detectors][sum_b M_b]; pinned memory

@@ -3,3 +3,4 @@ from .lloid_oracle import (  # noqa: F401
     N_DOWN, N_UP, Series, resample_kernel, decimate, upsample, upsample_input_range,
     basis_correlate, reconstruct, rate_groups, lloid_snr, brute_force, find_peaks,
 )
+from .events_oracle import find_peaks_overlap, template_acorr, xi2, coincidences, cluster  # noqa: F401,E402

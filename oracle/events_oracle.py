@@ -44,17 +44,19 @@ def find_peaks_overlap(rho: np.ndarray, buffer_len: int, overlap: int):
 
 
 def template_acorr(h_cos: np.ndarray, h_sin: np.ndarray, delta: int) -> np.ndarray:
-    """R[t + delta] = sum_m g[m] conj(g[m - t]) / sum_m |g[m]|^2 for t = -delta..delta, g = h_cos + i h_sin: the response
-    of the complex matched filter to its own template shifted by t, normalised so that R(0) = 1 exactly."""
+    """R[t + delta] = sum_m g[m] conj(g[m + t]) / sum_m |g[m]|^2 for t = -delta..delta, g = h_cos + i h_sin: what the
+    complex matched filter z[k] = sum_m g[m] d[k - N + 1 + m] returns t samples after the peak for its own template
+    (d = Re(conj(a) g) gives z[k0 + t] = a R[t] up to the template's negative-frequency content), normalised so that
+    R(0) = 1 exactly."""
     g = np.asarray(h_cos, dtype=np.float64) + 1j * np.asarray(h_sin, dtype=np.float64)
     N = len(g)
     norm = np.sum(np.abs(g) ** 2)
     R = np.zeros(2 * delta + 1, dtype=np.complex128)
     for t in range(-delta, delta + 1):
         if t >= 0:
-            R[t + delta] = np.sum(g[t:] * np.conj(g[:N - t])) if t < N else 0.0
+            R[t + delta] = np.sum(g[:N - t] * np.conj(g[t:])) if t < N else 0.0
         else:
-            R[t + delta] = np.sum(g[:N + t] * np.conj(g[-t:])) if -t < N else 0.0
+            R[t + delta] = np.sum(g[-t:] * np.conj(g[:N + t])) if -t < N else 0.0
     return R / norm
 
 
@@ -71,3 +73,48 @@ def xi2(z: np.ndarray, k0: int, acorr: np.ndarray) -> float:
     num = np.sum(np.abs(seg - z[k0] * acorr) ** 2)
     den = np.sum(2.0 - 2.0 * np.abs(acorr) ** 2)
     return float(num / den)
+
+
+def coincidences(snr: np.ndarray, sample: np.ndarray, dt: np.ndarray, threshold: float):
+    """Coincidence formation for ONE trigger window.
+
+    snr, sample: [n_det][M] single-detector triggers of the window (sample = integer trigger time in f0 samples on a
+    clock common to all detectors); dt: [n_det][n_det] symmetric coincidence windows in samples (light travel time +
+    0.005 s, rounded up); a trigger exists where snr >= threshold.
+    Per template: among all detector sets S with |S| >= 2 in which EVERY pair (a, b) has |sample_a - sample_b| <= dt[a][b],
+    the one with the largest network SNR^2 = sum_{a in S} snr_a^2 (ties: the smaller bit mask).  Returns
+    (mask [M] int -- bit a set for a participating detector, 0 = no coincidence --, net_snr [M])."""
+    snr = np.asarray(snr, dtype=np.float64)
+    sample = np.asarray(sample, dtype=np.int64)
+    n_det, M = snr.shape
+    mask = np.zeros(M, dtype=np.int64)
+    net = np.zeros(M)
+    subsets = [s for r in range(2, n_det + 1) for s in itertools.combinations(range(n_det), r)]
+    subsets.sort(key=lambda s: sum(1 << a for a in s))
+    for j in range(M):
+        best, best_mask = 0.0, 0
+        for s in subsets:
+            if any(snr[a, j] < threshold for a in s):
+                continue
+            if any(abs(int(sample[a, j]) - int(sample[b, j])) > dt[a][b] for a, b in itertools.combinations(s, 2)):
+                continue
+            v = sum(snr[a, j] ** 2 for a in s)
+            if v > best:
+                best, best_mask = v, sum(1 << a for a in s)
+        mask[j], net[j] = best_mask, math.sqrt(best)
+    return mask, net
+
+
+def cluster(mask: np.ndarray, net: np.ndarray, bank_off: Sequence[int]):
+    """Clustering: within each bank keep only the coincident event with the highest network SNR of the
+    window (ties: the lowest template index).  bank_off: [n_banks + 1] template offsets.  Returns per bank
+    (template index within the stream or -1, mask, net_snr)."""
+    out = []
+    for b in range(len(bank_off) - 1):
+        lo, hi = bank_off[b], bank_off[b + 1]
+        best, arg = 0.0, -1
+        for j in range(lo, hi):
+            if mask[j] != 0 and net[j] > best:
+                best, arg = net[j], j
+        out.append((arg, int(mask[arg]) if arg >= 0 else 0, float(best)))
+    return out

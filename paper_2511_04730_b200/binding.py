@@ -18,6 +18,10 @@ LLOID_OK, LLOID_EINVAL, LLOID_ELATENCY, LLOID_ENOMEM, LLOID_ECUDA, LLOID_ESTATE 
 LLOID_PREC_FP32_FFMA, LLOID_PREC_F16, LLOID_PREC_F16_SPLIT = 0, 1, 2
 
 PEAK_DTYPE = np.dtype([("snr", np.float32), ("sample", np.int32), ("phase", np.float32)])
+LLOID_MAX_DET = 4
+LLOID_NO_TRIGGER = -2147483648
+EVENT_DTYPE = np.dtype([("template_index", np.int32), ("det_mask", np.int32), ("net_snr", np.float32), ("reserved", np.int32),
+                        ("snr", np.float32, (LLOID_MAX_DET,)), ("sample", np.int32, (LLOID_MAX_DET,)), ("phase", np.float32, (LLOID_MAX_DET,))])
 
 
 class lloid_slice(C.Structure):
@@ -26,7 +30,8 @@ class lloid_slice(C.Structure):
 
 
 class lloid_options(C.Structure):
-    _fields_ = [("n_down", C.c_int32), ("n_up", C.c_int32), ("precision", C.c_int32), ("threshold", C.c_float)]
+    _fields_ = [("n_down", C.c_int32), ("n_up", C.c_int32), ("precision", C.c_int32), ("threshold", C.c_float),
+                ("trigger_overlap", C.c_int32)]
 
 
 class LloidError(RuntimeError):
@@ -49,6 +54,7 @@ def _load():
         "lloid_stream_destroy": (None, [vp]),
         "lloid_stream_push": (C.c_int, [vp, vp, vp, vp, i32]),
         "lloid_stream_push_host": (C.c_int, [vp, vp, vp]),
+        "lloid_stream_events": (C.c_int, [vp, vp, C.POINTER(i32), vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
         "lloid_stream_total_templates": (i32, [vp]),
@@ -68,7 +74,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_state_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
            "lloid_stage_name", "lloid_last_error", "lloid_version"]
@@ -94,7 +100,7 @@ def lloid_options_default() -> lloid_options:
 
 
 def lloid_bank_create(strain_rate_hz: int, n_templates: int, slices: Sequence[dict], precision: Optional[int] = None,
-                      threshold: float = 0.0, n_down: int = 32) -> int:
+                      threshold: float = 0.0, n_down: int = 32, trigger_overlap: int = 0) -> int:
     """slices: dicts with rate_hz, n_taps, n_basis, delay, basis (float32 [L][N]), recon (float32 [2M][L]);
     arrays are contiguous numpy arrays (host) or torch CUDA tensors (device).  Returns the bank handle."""
     arr = (lloid_slice * len(slices))()
@@ -114,6 +120,7 @@ def lloid_bank_create(strain_rate_hz: int, n_templates: int, slices: Sequence[di
     opt = lloid_options_default()
     opt.n_down = n_down
     opt.threshold = threshold
+    opt.trigger_overlap = trigger_overlap
     if precision is not None:
         opt.precision = precision
     h = C.c_void_p()
@@ -139,6 +146,11 @@ def lloid_stream_destroy(stream: int):
 def lloid_stream_push(stream: int, strain_ptr: int, peaks_ptr: int, snr_debug_ptr: int = 0, debug_bank: int = 0):
     """Raw device pointers (torch tensors' data_ptr())."""
     _check(_lib.lloid_stream_push(stream, strain_ptr, peaks_ptr, snr_debug_ptr or None, debug_bank))
+
+
+def lloid_stream_events(stream: int, peaks_ptr: int, dt_samples, events_ptr: int):
+    dt = np.ascontiguousarray(dt_samples, dtype=np.int32)
+    _check(_lib.lloid_stream_events(stream, peaks_ptr, dt.ctypes.data_as(C.POINTER(C.c_int32)), events_ptr))
 
 
 def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):
@@ -197,7 +209,8 @@ class LloidStream:
     """Owns bank and stream handles plus the torch device buffers a push needs."""
 
     def __init__(self, banks, n_detectors: int, buffer_len: int, precision: int = LLOID_PREC_F16_SPLIT,
-                 threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32, bank_handles=None, Ms=None):
+                 threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32, bank_handles=None, Ms=None,
+                 trigger_overlap: int = 0):
         """banks: iterable of Bank-like objects (uploaded here, owned by this object), or None with `bank_handles`
         (+ their template counts `Ms`): existing lloid_bank handles owned by the caller (several streams can share them)."""
         import torch
@@ -214,7 +227,7 @@ class LloidStream:
         else:
             for b in banks:                  # any iterable: a generator lets the caller build banks one at a time
                 self.Ms.append(b.M)
-                self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down))
+                self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down, trigger_overlap))
         self.cuda_stream = torch.cuda.current_stream(self.device)
         self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
         self.Mtot = lloid_stream_total_templates(self.handle)
@@ -242,6 +255,16 @@ class LloidStream:
         t.cuda.synchronize(self.device)
         peaks = self.peaks_dev.cpu().numpy().view(PEAK_DTYPE).reshape(self.n_det, self.Mtot)
         return (peaks, snr.cpu().numpy()) if snr is not None else peaks
+
+    def events(self, dt_samples, peaks_dev=None):
+        """Coincidence + clustering on the peaks of the last push (device): structured array [n_banks] (EVENT_DTYPE)."""
+        t = self.torch
+        if not hasattr(self, "events_dev"):
+            self.events_dev = t.zeros((len(self.bank_handles), EVENT_DTYPE.itemsize // 4), dtype=t.int32, device=self.device)
+        pk = self.peaks_dev if peaks_dev is None else peaks_dev
+        lloid_stream_events(self.handle, pk.data_ptr(), dt_samples, self.events_dev.data_ptr())
+        t.cuda.synchronize(self.device)
+        return self.events_dev.cpu().numpy().view(EVENT_DTYPE).reshape(len(self.bank_handles))
 
     def push_host(self):
         """End-to-end call on the pinned host buffers self.strain_host -> self.peaks_host (synchronous)."""

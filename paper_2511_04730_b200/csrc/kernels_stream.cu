@@ -375,8 +375,13 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
 // (strict '>' keeps the first maximum), then snr = sqrt(p), phase = atan2(im, re).
 // The last thread also advances the device-side stream clock n0 by B.
 // ------------------------------------------------------------------------------------------------
+// With overlapped trigger windows (Fig. 5) the window of a push is [n0 - overlap, n0 + B): `tail` holds, per
+// template, the peak of the PREVIOUS buffer's last `overlap` samples (index relative to that buffer); it competes with
+// the current buffer's peak (being earlier it wins a tie; reported sample = index - B < 0) and is then replaced by the
+// reduction of `tail_partial`, the current buffer's own tail peak.
 __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_det, int Mtot, int n_tt, int g,
-                                float threshold, lloid_peak *__restrict__ peaks, long long *n0, int B) {
+                                float threshold, lloid_peak *__restrict__ peaks, long long *n0, int B,
+                                PeakPartial *__restrict__ tail, const PeakPartial *__restrict__ tail_partial, int overlap) {
   // g (power of two <= 32) consecutive lanes share one template: coalesced reads of its n_tt partial peaks, then a
   // shuffle reduction.  "Better" = larger |z|^2, ties -> lower sample index (= the first maximum in time).
   const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
@@ -402,11 +407,22 @@ __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_d
     if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
   }
   if (!valid || li != 0) return;
+  if (tail != nullptr) {
+    const PeakPartial tp = tail[t];
+    if (tp.idx >= B - overlap && tp.idx < B && tp.p >= best.p) { best = tp; best.idx = tp.idx - B; }
+    PeakPartial nt;
+    nt.p = -3.f; nt.idx = 0x7fffffff; nt.re = 0.f; nt.im = 0.f;
+    for (int i = 0; i < 4; ++i) {
+      const PeakPartial c = tail_partial[(size_t)t * 4 + i];
+      if (c.p > nt.p || (c.p == nt.p && c.idx < nt.idx)) nt = c;
+    }
+    tail[t] = nt;
+  }
   lloid_peak o;
   o.snr = sqrtf(fmaxf(best.p, 0.f));
   o.sample = best.idx;
   o.phase = atan2f(best.im, best.re);
-  if (threshold > 0.f && o.snr < threshold) { o.snr = 0.f; o.sample = -1; o.phase = 0.f; }
+  if (threshold > 0.f && o.snr < threshold) { o.snr = 0.f; o.sample = LLOID_NO_TRIGGER; o.phase = 0.f; }
   peaks[t] = o;
 }
 
@@ -421,11 +437,12 @@ cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st)
 }
 
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
-                            lloid_peak *peaks, long long *n0, int B, cudaStream_t st) {
+                            lloid_peak *peaks, long long *n0, int B, PeakPartial *tail, const PeakPartial *tail_partial, int overlap,
+                            cudaStream_t st) {
   int g = 1;
   while (g < n_tt && g < 32) g <<= 1;
   const long long n = (long long)n_det * Mtot * g;
-  finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partial, n_det, Mtot, n_tt, g, threshold, peaks, n0, B);
+  finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partial, n_det, Mtot, n_tt, g, threshold, peaks, n0, B, tail, tail_partial, overlap);
   return cudaGetLastError();
 }
 

@@ -66,7 +66,7 @@ __global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                 int n_det, int B,
                 PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank,
-                int ring_off, int n_stages) {
+                int ring_off, int n_stages, int t_min) {
   constexpr int RBK = RES ? RBK_RES : RBK_STR;
   constexpr int RTILE_BYTES = TILE_M * RBK * 2;
   // Operand ring of K blocks of RBK (tiles of 128 rows x RBK fp16).  Streaming: NT = 3 * PLANES tiles
@@ -227,8 +227,8 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         __syncwarp();
         if (lane == 0) mbar_arrive(&tempty[buf]);
         // chunk maxima are independent; the running-maximum chain is one compare + select per chunk and the record
-        // stores are predicated (no vote / branch on the chain).  Only a buffer's last tile can be ragged: that case is
-        // a separate copy of the loop, chosen once per tile.
+        // stores are predicated (no vote / branch on the chain).  Only a buffer's last tile can be ragged: the masked
+        // loop is a separate copy, chosen once per tile.
         auto scan = [&](auto ragged_tag) {
           constexpr bool RAGGED = decltype(ragged_tag)::value;
 #pragma unroll
@@ -241,7 +241,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
                       __uint_as_float(vi[c * PK_CHUNK + i]), __uint_as_float(vi[c * PK_CHUNK + i + 1]), p[i], p[i + 1]);
             if (RAGGED) {
 #pragma unroll
-              for (int i = 0; i < PK_CHUNK; ++i) if (t0c + i >= B) p[i] = -1.f;
+              for (int i = 0; i < PK_CHUNK; ++i) if (t0c + i >= B || t0c + i < t_min) p[i] = -1.f;
             }
             float cm = p[0];
 #pragma unroll
@@ -258,7 +258,8 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
             }
           }
         };
-        if (tl.t0 + tt * TILE_N + TILE_N > B) scan(std::true_type()); else scan(std::false_type());
+        // (t_min > 0: the tail pass of the overlapped trigger windows looks at samples [t_min, B) only)
+        if (tl.t0 + tt * TILE_N + TILE_N > B || t_min > 0) scan(std::true_type()); else scan(std::false_type());
         if (dbg) {
           float *o = snr_debug + ((size_t)det * 2 * M + 2 * m) * B;
 #pragma unroll
@@ -563,6 +564,7 @@ struct TcPlan {
   int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
   TcReconTile *res_items_dev; int *res_begin_dev; int n_res_items, res_grid, res_ring_off, res_stages, str_stages;   // resident-R a3
+  TcReconTile *tail_dev; int *tail_begin_dev; int n_tail, tail_grid, tail_tmin;   // tail pass of overlapped trigger windows
   int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
@@ -665,7 +667,7 @@ void tc_plan_destroy(TcPlan *p) {
 }
 
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
-                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes) {
+                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes, int overlap) {
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
@@ -757,6 +759,18 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
       }
     }
   }
+  // tail pass (trigger windows overlapped by `overlap` samples): one streaming item per (bank, template
+  // tile, detector) over the tiles that hold the buffer's last `overlap` samples; its epilogue masks samples < B - overlap
+  std::vector<TcReconTile> tail;
+  p->tail_tmin = std::max(0, B - overlap);
+  if (overlap > 0) {
+    const int i0 = p->tail_tmin / TILE_N;
+    for (size_t b = 0; b < banks.size(); ++b)
+      for (int m0 = 0; m0 < banks[b].M; m0 += TILE_M)
+        for (int det = 0; det < n_det; ++det) tail.push_back({(int)b, det, 1, m0, i0 * TILE_N, ntile - i0, 0});
+  }
+  p->n_tail = (int)tail.size();
+  p->tail_grid = std::max(1, std::min(p->n_tail, sms));
   p->n_res_items = (int)ri.size();
   p->res_grid = std::max(1, std::min(p->n_res_items, sms));
   p->res_ring_off = ((res_kmax + RBK_RES - 1) / RBK_RES) * 4 * TILE_M * RBK_RES * 2;
@@ -773,8 +787,10 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   lpt_assign(ri, p->res_grid, [&](const TcReconTile &t) {
     const long long kp = rb[t.bank].Kpad;
     return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 388, 600) + 3000 + kp * 8; }, ibegin);
+  std::vector<int> tbegin;
+  lpt_assign(tail, p->tail_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, tbegin);
   if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->res_items_dev, ri) ||
-      !plan_upload(p, &p->res_begin_dev, ibegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+      !plan_upload(p, &p->res_begin_dev, ibegin) || !plan_upload(p, &p->tail_dev, tail) || !plan_upload(p, &p->tail_begin_dev, tbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   p->recon_smem = RECON_SMEM_BUDGET + 1024 + 256;
@@ -803,22 +819,34 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
 }
 
 int tc_plan_n_tt(const TcPlan *p) { return p->n_tt; }
-int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_res_items ? 1 : 0); }
+int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_res_items ? 1 : 0) + (p->n_tail ? 1 : 0); }
+
+// tail pass: the peak of every template over the buffer's last `overlap` samples -> tail_partial [n_det][Mtot][4]
+cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st) {
+  if (p->n_tail == 0) return cudaSuccess;
+  if (p->planes == 2)
+    recon_tc_kernel<2, false><<<p->tail_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->tail_dev, p->tail_begin_dev, p->n_det, p->B,
+                                                                               tail_partial, Mtot, 4, nullptr, -1, 0, p->str_stages, p->tail_tmin);
+  else
+    recon_tc_kernel<1, false><<<p->tail_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->tail_dev, p->tail_begin_dev, p->n_det, p->B,
+                                                                               tail_partial, Mtot, 4, nullptr, -1, 0, p->str_stages, p->tail_tmin);
+  return cudaGetLastError();
+}
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
   if (p->n_res_items) {
     recon_tc_kernel<2, true><<<p->res_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->res_items_dev, p->res_begin_dev, p->n_det, p->B,
-                                                                              partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off, p->res_stages);
+                                                                              partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off, p->res_stages, 0);
     cudaError_t e0 = cudaGetLastError();
     if (e0 != cudaSuccess) return e0;
   }
   if (p->n_rtiles == 0) return cudaSuccess;
   if (p->planes == 2)
     recon_tc_kernel<2, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages);
+                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
   else
     recon_tc_kernel<1, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages);
+                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
   return cudaGetLastError();
 }
 

@@ -34,6 +34,7 @@ extern "C" void lloid_options_default(lloid_options *opt) {
   opt->n_up = LLOID_NUP;
   opt->precision = LLOID_PREC_F16_SPLIT;
   opt->threshold = 0.f;
+  opt->trigger_overlap = 0;
 }
 
 extern "C" void lloid_bank_destroy(lloid_bank *b) {
@@ -53,6 +54,9 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
   lloid_options_default(&opt);
   if (opt_in) opt = *opt_in;
   if (opt.n_up != LLOID_NUP) { set_error("bank_create: only n_up = %d is supported", LLOID_NUP); return LLOID_EINVAL; }
+  if (opt.trigger_overlap < 0 || (opt.trigger_overlap > 0 && opt.precision == LLOID_PREC_FP32_FFMA)) {
+    set_error("bank_create: trigger_overlap must be >= 0 and needs a tensor-core precision"); return LLOID_EINVAL;
+  }
   if (opt.n_down < 1 || opt.n_down > 64) { set_error("bank_create: n_down %d outside [1, 64]", opt.n_down); return LLOID_EINVAL; }
   if (opt.precision < LLOID_PREC_FP32_FFMA || opt.precision > LLOID_PREC_F16_SPLIT) {
     set_error("bank_create: unknown precision %d", opt.precision); return LLOID_EINVAL;

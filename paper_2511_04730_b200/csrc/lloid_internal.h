@@ -116,19 +116,24 @@ cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_m
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
 cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st);
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
-                            lloid_peak *peaks, long long *n0, int B, cudaStream_t st);
+                            lloid_peak *peaks, long long *n0, int B, PeakPartial *tail, const PeakPartial *tail_partial, int overlap,
+                            cudaStream_t st);
+
+cudaError_t launch_coinc_cluster(const lloid_peak *peaks, int n_det, int Mtot, const int *bank_off_dev, int n_banks,
+                                 const int32_t *dt_host, lloid_event *events, cudaStream_t st);   // lloid_events.cu
 
 // ---------------------------------------------------------------------------------------------- tcgen05 path (kernels_tc.cu)
 struct TcPlan;
 int tc_time_splits(int B, long long n_mtile_units);   // n_mtile_units = sum_banks ceil(M/128) * n_det
 int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel for a slice of Npad taps   // partial peaks per template written by the tensor-core a3 kernel
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
-                   const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes);
+                   const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes, int overlap);
 void tc_plan_destroy(TcPlan *p);
 int tc_plan_n_tt(const TcPlan *p);              // partial peaks per template and detector the a3 kernels write
 int tc_plan_recon_launches(const TcPlan *p);    // 1 or 2: streaming kernel and / or resident-R kernel
 cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st);
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank,
                             cudaStream_t st);
+cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st);
 
 }  // namespace lloid

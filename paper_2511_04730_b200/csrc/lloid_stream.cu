@@ -16,7 +16,9 @@ using namespace lloid;
 
 struct lloid_stream {
   std::vector<const lloid_bank *> banks;
-  int n_det, B, f0, precision, n_down, Mtot, n_tt, max_mtiles;
+  int n_det, B, f0, precision, n_down, Mtot, n_tt, max_mtiles, overlap;
+  int *bank_off_dev;                               // [n_banks + 1] template offsets (coincidence / clustering)
+  PeakPartial *tail_dev, *tail_partial_dev;        // overlapped trigger windows: previous buffer's tail peak, this buffer's partials
   float threshold;
   cudaStream_t st;
   long long n0_host;
@@ -99,17 +101,20 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   for (int b = 0; b < n_banks; ++b) {
     if (!banks[b]) { set_error("stream_create: bank %d is NULL", b); return LLOID_EINVAL; }
     if (banks[b]->f0 != banks[0]->f0 || banks[b]->opt.precision != banks[0]->opt.precision ||
-        banks[b]->opt.n_down != banks[0]->opt.n_down || banks[b]->opt.threshold != banks[0]->opt.threshold) {
-      set_error("stream_create: bank %d differs from bank 0 in strain rate, precision, n_down or threshold", b); return LLOID_EINVAL;
+        banks[b]->opt.n_down != banks[0]->opt.n_down || banks[b]->opt.threshold != banks[0]->opt.threshold ||
+        banks[b]->opt.trigger_overlap != banks[0]->opt.trigger_overlap) {
+      set_error("stream_create: bank %d differs from bank 0 in strain rate, precision, n_down, threshold or trigger_overlap", b); return LLOID_EINVAL;
     }
     for (const SliceInfo &si : banks[b]->slices) Dmax = std::max(Dmax, si.D);
   }
+  if (banks[0]->opt.trigger_overlap >= B) { set_error("stream_create: trigger_overlap %d must be smaller than buffer_len %d", banks[0]->opt.trigger_overlap, B); return LLOID_EINVAL; }
   if (B % Dmax != 0) { set_error("stream_create: buffer_len %d is not a multiple of the largest decimation factor %d", B, Dmax); return LLOID_EINVAL; }
   lloid_stream *s = new (std::nothrow) lloid_stream();
   if (!s) { set_error("stream_create: out of host memory"); return LLOID_ENOMEM; }
   s->banks.assign(banks, banks + n_banks);
   s->n_det = n_det; s->B = B; s->f0 = banks[0]->f0; s->precision = banks[0]->opt.precision;
-  s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold;
+  s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold; s->overlap = banks[0]->opt.trigger_overlap;
+  s->tail_dev = nullptr; s->tail_partial_dev = nullptr;
   s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false; s->failed = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
@@ -334,11 +339,17 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   CK(dev_upload(s, &s->items_dev, items));
   CK(dev_upload(s, &s->uprows_dev, uprows));
   CK(dev_upload(s, &s->rbanks_dev, s->rbanks));
+  {
+    std::vector<int> off;
+    for (const ReconBank &rb : s->rbanks) off.push_back(rb.tmpl_off);
+    off.push_back(s->Mtot);
+    CK(dev_upload(s, &s->bank_off_dev, off));
+  }
   s->n_tt = (B + 63) / 64;
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
   if (s->precision != LLOID_PREC_FP32_FFMA) {
-    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes);
+    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
     s->n_tt = tc_plan_n_tt(s->tc);                 // partial peaks per template: the larger of the two a3 kernels' splits
     s->work[0] *= (planes == 2 ? 2 : 1);           // split mode: two MMAs per product in a2 (U_hi x, U_lo x) and in a3
@@ -347,6 +358,12 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   // partial-peak slots a kernel never writes hold p = -3 (below every real partial, finalize ignores them)
   CK(dev_alloc(s, &s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt));
   CK(launch_fill_partial(s->partial_dev, (size_t)n_det * s->Mtot * s->n_tt, s->st));
+  if (s->overlap > 0) {
+    // zeroed tail state = "no tail peak" (index 0 lies outside the overlap): reset restores it
+    CK(dev_alloc(s, &s->tail_dev, (size_t)n_det * s->Mtot, true));
+    CK(dev_alloc(s, &s->tail_partial_dev, (size_t)n_det * s->Mtot * 4));
+    CK(launch_fill_partial(s->tail_partial_dev, (size_t)n_det * s->Mtot * 4, s->st));
+  }
   CK(cudaDeviceSynchronize());
   *out = s;
   return LLOID_OK;
@@ -389,10 +406,12 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
     else e = launch_recon_ffma(s->rbanks_dev, (int)s->banks.size(), s->max_mtiles, s->n_det, s->B, s->partial_dev,
                                s->Mtot, snr_debug, snr_debug ? debug_bank : -1, s->st);
   }
+  if (e == cudaSuccess && s->overlap > 0) e = tc_launch_recon_tail(s->tc, s->tail_partial_dev, s->Mtot, s->st);
   mark(4);
   if (e == cudaSuccess) where = "a5 finalize";
   if (e == cudaSuccess)
-    e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->st);
+    e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->tail_dev,
+                        s->tail_partial_dev, s->overlap, s->st);
   mark(5);
   if (s->stage_timing) s->ev_rec.push_back(std::move(ev));
   if (e != cudaSuccess) {
@@ -402,6 +421,19 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
     set_error("stream_push: launch of %s failed: %s (stream needs lloid_state_reset)", where, cudaGetErrorString(e)); return LLOID_ECUDA;
   }
   s->n0_host += s->B;
+  return LLOID_OK;
+}
+
+extern "C" int lloid_stream_events(lloid_stream *s, const lloid_peak *peaks, const int32_t *dt_samples, lloid_event *events) {
+  if (!s || !peaks || !dt_samples || !events) { set_error("stream_events: NULL argument"); return LLOID_EINVAL; }
+  if (s->n_det > LLOID_MAX_DET) { set_error("stream_events: at most %d detectors", LLOID_MAX_DET); return LLOID_EINVAL; }
+  for (int a = 0; a < s->n_det; ++a)
+    for (int c = 0; c < s->n_det; ++c)
+      if (dt_samples[a * s->n_det + c] < 0 || dt_samples[a * s->n_det + c] != dt_samples[c * s->n_det + a]) {
+        set_error("stream_events: dt_samples must be symmetric and non-negative"); return LLOID_EINVAL;
+      }
+  cudaError_t e = launch_coinc_cluster(peaks, s->n_det, s->Mtot, s->bank_off_dev, (int)s->banks.size(), dt_samples, events, s->st);
+  if (e != cudaSuccess) { set_error("stream_events: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   return LLOID_OK;
 }
 

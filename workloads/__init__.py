@@ -18,6 +18,7 @@ from .lloid_inputs import (  # noqa: F401
     decompose_slice,
     injection_waveform,
     random_bank,
+    random_triggers,
     make_strain,
     inject,
     make_config,

@@ -396,3 +396,23 @@ CONFIGS = {
 
 def make_config(number: int, **overrides) -> Config:
     return dataclasses.replace(CONFIGS[number], **overrides)
+
+
+def random_triggers(seed: int, n_det: int, M: int, buffer_len: int, p_trigger: float = 0.5, p_coinc: float = 0.3,
+                    max_shift: int = 40, overlap: int = 0):
+    """Seeded synthetic single-detector triggers [n_det][M] for the coincidence / clustering stage (input generator only):
+    structured array (snr float32, sample int32, phase float32); sample = NO_TRIGGER (-2^31) where there is no trigger.
+    A fraction p_coinc of the templates gets triggers at nearly equal times in several detectors."""
+    rng = np.random.default_rng(seed)
+    dt = np.dtype([("snr", np.float32), ("sample", np.int32), ("phase", np.float32)])
+    out = np.zeros((n_det, M), dtype=dt)
+    out["sample"] = -2147483648
+    for j in range(M):
+        base = int(rng.integers(-overlap, buffer_len))
+        coinc = rng.random() < p_coinc
+        for a in range(n_det):
+            if rng.random() < p_trigger:
+                k = base + int(rng.integers(-max_shift, max_shift + 1)) if coinc else int(rng.integers(-overlap, buffer_len))
+                k = min(max(k, -overlap), buffer_len - 1)
+                out[a, j] = (np.float32(4.0 + 8.0 * rng.random()), k, np.float32(rng.uniform(-np.pi, np.pi)))
+    return out
