@@ -128,6 +128,20 @@ int lloid_stream_push(lloid_stream *stream, const float *strain, lloid_peak *pea
  * Errors: EINVAL (null pointer, more than LLOID_MAX_DET detectors, negative window), ECUDA. */
 int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int32_t *dt_samples, lloid_event *events);
 
+/* Signal-based consistency statistic xi^2 of Eq. 10 for the triggers of ONE bank whose SNR series is
+ * materialised in device memory (the snr_debug output of lloid_stream_push; the caller keeps consecutive buffers side by
+ * side so that the +-delta samples around a trigger are present -- the padding of Fig. 5 -- and calls this one buffer
+ * later).  Asynchronous on cuda_stream.
+ *   snr             DEVICE, [2*n_templates][n_samples] fp32, row 2j real, 2j+1 imaginary part of z_j
+ *   trigger_sample  DEVICE, [n_templates] index of the trigger in [0, n_samples), LLOID_NO_TRIGGER = none
+ *   acorr           DEVICE, [n_templates][2*delta+1][2] fp32 (re, im): R_j(t), t = -delta..delta, R_j(0) = 1,
+ *                   R_j(t) = sum_m g[m] conj(g[m+t]) / sum |g|^2 for the complex template g = h_2j + i h_2j+1
+ *   delta           half width in samples: (autocorrelation length - 1) / 2, 175 or 350 in the paper
+ *   xi2_out         DEVICE, [n_templates] fp32; -1 where there is no trigger.  Samples outside [0, n_samples) count as 0.
+ * Errors: EINVAL, ECUDA. */
+int lloid_xi2_series(const float *snr, int32_t n_templates, int64_t n_samples, const int32_t *trigger_sample,
+                     const float *acorr, int32_t delta, float *xi2_out, void *cuda_stream);
+
 /* Same through HOST buffers: copies strain host->device, pushes, copies peaks device->host and waits for
  * the stream.  strain_host [n_detectors][buffer_len], peaks_host [n_detectors][sum_b M_b]; pinned memory
  * makes the copies asynchronous but is not required. */

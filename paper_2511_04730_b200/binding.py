@@ -55,6 +55,7 @@ def _load():
         "lloid_stream_push": (C.c_int, [vp, vp, vp, vp, i32]),
         "lloid_stream_push_host": (C.c_int, [vp, vp, vp]),
         "lloid_stream_events": (C.c_int, [vp, vp, C.POINTER(i32), vp]),
+        "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
         "lloid_stream_total_templates": (i32, [vp]),
@@ -74,7 +75,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_state_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
            "lloid_stage_name", "lloid_last_error", "lloid_version"]
@@ -151,6 +152,17 @@ def lloid_stream_push(stream: int, strain_ptr: int, peaks_ptr: int, snr_debug_pt
 def lloid_stream_events(stream: int, peaks_ptr: int, dt_samples, events_ptr: int):
     dt = np.ascontiguousarray(dt_samples, dtype=np.int32)
     _check(_lib.lloid_stream_events(stream, peaks_ptr, dt.ctypes.data_as(C.POINTER(C.c_int32)), events_ptr))
+
+
+def lloid_xi2_series(snr_dev, trigger_sample_dev, acorr_dev, delta: int, cuda_stream: int = 0):
+    """torch CUDA tensors: snr float32 [2M][n], trigger_sample int32 [M], acorr float32 [M][2 delta + 1][2] -> xi2 float32 [M]."""
+    import torch
+    M, n = snr_dev.shape[0] // 2, snr_dev.shape[1]
+    assert snr_dev.is_contiguous() and acorr_dev.is_contiguous() and tuple(acorr_dev.shape) == (M, 2 * delta + 1, 2)
+    out = torch.empty(M, dtype=torch.float32, device=snr_dev.device)
+    _check(_lib.lloid_xi2_series(snr_dev.data_ptr(), M, n, trigger_sample_dev.data_ptr(), acorr_dev.data_ptr(), delta, out.data_ptr(),
+                                 cuda_stream))
+    return out
 
 
 def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):

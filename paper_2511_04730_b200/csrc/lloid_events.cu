@@ -98,3 +98,53 @@ cudaError_t launch_coinc_cluster(const lloid_peak *peaks, int n_det, int Mtot, c
 }
 
 }  // namespace lloid
+
+// ------------------------------------------------------------------------------------------------
+// Signal-based consistency test, Eq. 10, for the triggers of one bank whose SNR series is
+// materialised (the snr_debug output of lloid_stream_push, consecutive buffers side by side):
+//   xi2_j = sum_{t=-delta}^{delta} |z_j[k0 + t] - z_j[k0] R_j[t]|^2 / sum_t (2 - 2 |R_j[t]|^2)
+// One warp per template; lane l takes t = -delta + l, -delta + l + 32, ...; fixed-order shuffle reduction
+// (deterministic).  Samples outside [0, n) count as zero (stream start / the caller did not wait for the padding).
+// ------------------------------------------------------------------------------------------------
+namespace lloid {
+
+__global__ void __launch_bounds__(256) xi2_series_kernel(const float *__restrict__ snr, int M, long long n,
+                                                         const int *__restrict__ k0v, const float2 *__restrict__ acorr, int delta,
+                                                         float *__restrict__ out) {
+  const int j = (int)((blockIdx.x * (long long)blockDim.x + threadIdx.x) >> 5), lane = threadIdx.x & 31;
+  if (j >= M) return;
+  const int k0 = k0v[j];
+  if (k0 == LLOID_NO_TRIGGER || k0 < 0 || k0 >= n) { if (lane == 0) out[j] = -1.f; return; }
+  const float *re = snr + (size_t)(2 * j) * n, *im = re + n;
+  const float2 *R = acorr + (size_t)j * (2 * delta + 1);
+  const float z0r = re[k0], z0i = im[k0];
+  float num = 0.f, den = 0.f;
+  for (int u = lane; u <= 2 * delta; u += 32) {
+    const long long k = (long long)k0 - delta + u;
+    const float2 a = R[u];
+    float zr = 0.f, zi = 0.f;
+    if (k >= 0 && k < n) { zr = re[k]; zi = im[k]; }
+    const float dr = zr - (z0r * a.x - z0i * a.y), di = zi - (z0r * a.y + z0i * a.x);
+    num += dr * dr + di * di;
+    den += 2.f - 2.f * (a.x * a.x + a.y * a.y);
+  }
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) { num += __shfl_xor_sync(0xffffffffu, num, o); den += __shfl_xor_sync(0xffffffffu, den, o); }
+  if (lane == 0) out[j] = num / den;
+}
+
+}  // namespace lloid
+
+extern "C" int lloid_xi2_series(const float *snr, int32_t n_templates, int64_t n_samples, const int32_t *trigger_sample,
+                                const float *acorr, int32_t delta, float *xi2_out, void *cuda_stream) {
+  using namespace lloid;
+  if (!snr || !trigger_sample || !acorr || !xi2_out || n_templates < 1 || n_samples < 1 || delta < 1) {
+    set_error("xi2_series: NULL pointer or non-positive size"); return LLOID_EINVAL;
+  }
+  const long long threads = (long long)n_templates * 32;
+  xi2_series_kernel<<<(unsigned)((threads + 255) / 256), 256, 0, (cudaStream_t)cuda_stream>>>(
+      snr, n_templates, n_samples, trigger_sample, reinterpret_cast<const float2 *>(acorr), delta, xi2_out);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) { set_error("xi2_series: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  return LLOID_OK;
+}

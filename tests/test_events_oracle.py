@@ -157,3 +157,12 @@ def test_cluster_keeps_one_event_per_bank():
     net = np.array([0.0, 9.0, 11.0, 0.0, 0.0, 0.0, 8.0, 12.0, 12.0])
     out = cluster(mask, net, [0, 3, 6, 9])
     assert out == [(2, 5, 11.0), (-1, 0, 0.0), (7, 3, 12.0)]      # tie in the last bank -> the lower template index
+
+
+def test_generator_autocorrelations_equal_the_oracle_definition():
+    """workloads.template_autocorrelations (numpy.correlate, feeds the CUDA side) against oracle.template_acorr."""
+    from workloads import chirp_templates, template_autocorrelations
+    H = chirp_templates([1.1, 1.7, 2.9], 1.0, 2048, 1024.0)
+    A = template_autocorrelations(H, 175)
+    for j in range(3):
+        assert np.abs(A[j] - template_acorr(H[2 * j], H[2 * j + 1], 175)).max() < 1e-13

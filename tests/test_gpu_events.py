@@ -150,3 +150,50 @@ def test_end_to_end_three_detector_event():
     e = evs[5][1]
     assert e["template_index"] == 24 + 17 and e["det_mask"] == 7 and e["net_snr"] > 11
     assert e["sample"][1] < 0 <= e["sample"][0]
+
+
+def test_xi2_from_the_materialised_snr_against_the_oracle():
+    """Eq. 10 on the GPU SNR series (snr_debug dumps of consecutive buffers side by side) for the triggers of every middle
+    buffer, against oracle.xi2 on the float64 LLOID SNR at the oracle's own trigger samples."""
+    torch = _cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import find_peaks, lloid_snr, xi2
+    from workloads import bank_from_layout, chirp_templates, inject, injection_waveform, make_strain, template_autocorrelations
+    f0, B, delta = 2048, 1024, 175
+    mc = np.linspace(1.2, 1.4, 21)
+    lay = [(2048, 0, 1024), (1024, 1024, 3072), (512, 3072, 8192), (256, 8192, 16384)]
+    bank = bank_from_layout(mc, 8.0, lay, f0=f0).as_f32()
+    n_push = 20
+    strain = make_strain(91, n_push * B)[None].copy()
+    inject(strain[0], injection_waveform(float(mc[7]), 8.0, 14.0, 1.1, f0), 18 * B + 300)
+    acorr = template_autocorrelations(chirp_templates(mc, 8.0, f0, 1024.0), delta)
+    st = lib.LloidStream([bank], 1, B)
+    snr_all = torch.zeros((2 * bank.M, n_push * B), dtype=torch.float32, device="cuda")
+    pks = []
+    for p in range(n_push):
+        pk, snr = st.push(strain[:, p * B:(p + 1) * B], want_snr_bank=0)
+        snr_all[:, p * B:(p + 1) * B] = torch.from_numpy(snr[0]).cuda()
+        pks.append(pk[0].copy())
+    st.close()
+    ac_dev = torch.from_numpy(np.stack([acorr.real, acorr.imag], axis=-1).astype(np.float32)).cuda().contiguous()
+    ref = lloid_snr(bank, strain[0])
+    z = ref[0::2] + 1j * ref[1::2]
+    _, idx_o, _ = find_peaks(ref, B)
+    worst, n_cmp = 0.0, 0
+    for p in (1, 9, 17, 18):
+        k0 = (pks[p]["sample"].astype(np.int64) + p * B).astype(np.int32)
+        got = lib.binding.lloid_xi2_series(snr_all, torch.from_numpy(k0).cuda(), ac_dev, delta).cpu().numpy()
+        for j in range(bank.M):
+            if pks[p]["sample"][j] != idx_o[p, j]:
+                continue                                    # a near-tie resolved differently: another trigger, not comparable
+            want = xi2(z[j], int(idx_o[p, j]) + p * B, acorr[j])
+            worst = max(worst, abs(got[j] - want) / want)
+            n_cmp += 1
+    print(f"xi2: {n_cmp} triggers compared, worst relative error {worst:.2e}")
+    assert n_cmp > 70 and worst < 2e-3
+    # the injected template's trigger is consistent with its autocorrelation; all values are O(1) in noise
+    got18 = lib.binding.lloid_xi2_series(snr_all, torch.from_numpy((pks[18]["sample"].astype(np.int64) + 18 * B).astype(np.int32)).cuda(),
+                                         ac_dev, delta).cpu().numpy()
+    assert pks[18]["snr"][7] > 11 and 0.3 < got18[7] < 2.5
+    none = torch.full((bank.M,), NO_TRIGGER, dtype=torch.int32, device="cuda")
+    assert (lib.binding.lloid_xi2_series(snr_all, none, ac_dev, delta).cpu().numpy() == -1).all()

@@ -19,6 +19,7 @@ from .lloid_inputs import (  # noqa: F401
     injection_waveform,
     random_bank,
     random_triggers,
+    template_autocorrelations,
     make_strain,
     inject,
     make_config,

@@ -416,3 +416,23 @@ def random_triggers(seed: int, n_det: int, M: int, buffer_len: int, p_trigger: f
                 k = min(max(k, -overlap), buffer_len - 1)
                 out[a, j] = (np.float32(4.0 + 8.0 * rng.random()), k, np.float32(rng.uniform(-np.pi, np.pi)))
     return out
+
+
+def template_autocorrelations(H: np.ndarray, delta: int) -> np.ndarray:
+    """Input generator for the xi^2 test: [M][2 delta + 1] complex128 autocorrelations of the complex
+    templates g_j = H[2j] + i H[2j+1], R_j(t) = sum_m g_j[m] conj(g_j[m + t]) / sum |g_j|^2, t = -delta..delta, through
+    numpy's correlate (R_j(0) = 1)."""
+    H = np.asarray(H, dtype=np.float64)
+    M, N = H.shape[0] // 2, H.shape[1]
+    out = np.zeros((M, 2 * delta + 1), dtype=np.complex128)
+    for j in range(M):
+        g = H[2 * j] + 1j * H[2 * j + 1]
+        # np.correlate(a, v, "full")[k] = sum_n a[n + k - (N - 1)] conj(v[n]); lag t = -(k - (N - 1))
+        c = np.correlate(g, g, mode="full")
+        mid = N - 1
+        lags = np.arange(-delta, delta + 1)
+        idx = mid - lags
+        ok = (idx >= 0) & (idx < len(c))
+        out[j, ok] = c[idx[ok]]
+        out[j] /= np.sum(np.abs(g) ** 2)
+    return out
