@@ -142,6 +142,27 @@ int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int
 int lloid_xi2_series(const float *snr, int32_t n_templates, int64_t n_samples, const int32_t *trigger_sample,
                      const float *acorr, int32_t delta, float *xi2_out, void *cuda_stream);
 
+/* PSD estimation + whitening front end (Figs. 2-3), the step before the path.  Per detector and push:
+ * the newest fft_len - 2 zero_pad input samples times a Hann window, zero padded to fft_len -> FFT -> per bin the median of
+ * the last n_median instantaneous PSDs updates a running geometric mean over n_average blocks (PSD = its arithmetic-mean
+ * equivalent) -> divide by sqrt(PSD), drop the bins above rate_out / 2 (frequency-domain downsampling) -> inverse FFT ->
+ * Tukey window (tapers of zero_pad) -> overlap-add.  One push takes hop_in = fft_len / 2 - zero_pad samples at rate_in and
+ * returns hop_out = hop_in * rate_out / rate_in samples at rate_out of unit variance, lagging the input by fft_len / 2
+ * input samples.  Paper values: rate_in 16384, rate_out 2048, fft_len 4 s, zero_pad 1 s, n_median 7.  Zero history at
+ * start; gaps and gating are not handled.  The FFTs are cuFFT transforms (libcufft.so.11 is loaded at create).
+ *   strain_in  DEVICE [n_detectors][hop_in] fp32        white_out  DEVICE [n_detectors][hop_out] fp32
+ *   psd_out    DEVICE [n_detectors][psd_bins] fp32 one-sided PSD per Hz at bin k * rate_in / fft_len, or NULL
+ * Errors: EINVAL (sizes), ENOMEM, ECUDA (cuFFT missing or failing, launch failure). */
+typedef struct lloid_whitener lloid_whitener;
+int lloid_whitener_create(lloid_whitener **out, int32_t n_detectors, int32_t rate_in, int32_t rate_out, int32_t fft_len,
+                          int32_t zero_pad, int32_t n_median, int32_t n_average, void *cuda_stream);
+int lloid_whitener_push(lloid_whitener *w, const float *strain_in, float *white_out, float *psd_out);
+int lloid_whitener_reset(lloid_whitener *w);
+void lloid_whitener_destroy(lloid_whitener *w);
+int32_t lloid_whitener_hop_in(const lloid_whitener *w);
+int32_t lloid_whitener_hop_out(const lloid_whitener *w);
+int32_t lloid_whitener_psd_bins(const lloid_whitener *w);
+
 /* Same through HOST buffers: copies strain host->device, pushes, copies peaks device->host and waits for
  * the stream.  strain_host [n_detectors][buffer_len], peaks_host [n_detectors][sum_b M_b]; pinned memory
  * makes the copies asynchronous but is not required. */

@@ -4,3 +4,4 @@ from .lloid_oracle import (  # noqa: F401
     basis_correlate, reconstruct, rate_groups, lloid_snr, brute_force, find_peaks,
 )
 from .events_oracle import find_peaks_overlap, template_acorr, xi2, coincidences, cluster  # noqa: F401,E402
+from .whiten_oracle import Whitener, log_median_mean, hann_periodic, tukey_taper  # noqa: F401,E402

@@ -4,4 +4,4 @@ The product is the C-ABI library ``liblloid.so`` (include/lloid.h, sources in cs
 ctypes binding.  Import fails loudly when the library has not been built -- there is no CPU fallback.
 """
 from .binding import *  # noqa: F401,F403
-from .binding import (EXPORTS, LIB_PATH, PEAK_DTYPE, LloidError, LloidStream, bank_slices)  # noqa: F401
+from .binding import (EXPORTS, LIB_PATH, PEAK_DTYPE, LloidError, LloidStream, Whitener, bank_slices)  # noqa: F401

@@ -55,6 +55,13 @@ def _load():
         "lloid_stream_push": (C.c_int, [vp, vp, vp, vp, i32]),
         "lloid_stream_push_host": (C.c_int, [vp, vp, vp]),
         "lloid_stream_events": (C.c_int, [vp, vp, C.POINTER(i32), vp]),
+        "lloid_whitener_create": (C.c_int, [C.POINTER(vp), i32, i32, i32, i32, i32, i32, i32, vp]),
+        "lloid_whitener_push": (C.c_int, [vp, vp, vp, vp]),
+        "lloid_whitener_reset": (C.c_int, [vp]),
+        "lloid_whitener_destroy": (None, [vp]),
+        "lloid_whitener_hop_in": (i32, [vp]),
+        "lloid_whitener_hop_out": (i32, [vp]),
+        "lloid_whitener_psd_bins": (i32, [vp]),
         "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
@@ -75,7 +82,8 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_state_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
+           "lloid_whitener_destroy", "lloid_whitener_hop_in", "lloid_whitener_hop_out", "lloid_whitener_psd_bins", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
            "lloid_stage_name", "lloid_last_error", "lloid_version"]
@@ -215,6 +223,41 @@ def bank_slices(bank) -> List[dict]:
     return [dict(rate_hz=s.rate, n_taps=s.n_taps, n_basis=s.U.shape[0], delay=s.delay,
                  basis=np.ascontiguousarray(s.U, dtype=np.float32), recon=np.ascontiguousarray(s.R, dtype=np.float32))
             for s in bank.slices]
+
+
+class Whitener:
+    """PSD estimation + whitening front end (lloid_whitener_*): torch CUDA tensors in and out."""
+
+    def __init__(self, n_detectors: int, rate_in: int, rate_out: int, fft_len: int, zero_pad: int, n_median: int = 7,
+                 n_average: int = 64, device: str = "cuda:0"):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("Whitener needs a CUDA device (no CPU fallback)")
+        self.torch, self.device = torch, torch.device(device)
+        torch.cuda.set_device(self.device)
+        h = C.c_void_p()
+        _check(_lib.lloid_whitener_create(C.byref(h), n_detectors, rate_in, rate_out, fft_len, zero_pad, n_median, n_average,
+                                          torch.cuda.current_stream(self.device).cuda_stream))
+        self.handle, self.n_det = h.value, n_detectors
+        self.hop_in, self.hop_out = _lib.lloid_whitener_hop_in(h), _lib.lloid_whitener_hop_out(h)
+        self.psd_bins = _lib.lloid_whitener_psd_bins(h)
+
+    def push(self, strain_dev, want_psd: bool = False):
+        t = self.torch
+        assert strain_dev.is_cuda and strain_dev.dtype == t.float32 and strain_dev.is_contiguous()
+        assert tuple(strain_dev.shape) == (self.n_det, self.hop_in)
+        out = t.empty((self.n_det, self.hop_out), dtype=t.float32, device=self.device)
+        psd = t.empty((self.n_det, self.psd_bins), dtype=t.float32, device=self.device) if want_psd else None
+        _check(_lib.lloid_whitener_push(self.handle, strain_dev.data_ptr(), out.data_ptr(), psd.data_ptr() if want_psd else None))
+        return (out, psd) if want_psd else out
+
+    def reset(self):
+        _check(_lib.lloid_whitener_reset(self.handle))
+
+    def close(self):
+        if self.handle:
+            _lib.lloid_whitener_destroy(self.handle)
+            self.handle = None
 
 
 class LloidStream:
