@@ -31,7 +31,7 @@ if ROOT not in sys.path:
 METRIC = "template*detector*data-seconds filtered per wall-second"
 UNIT = "template*detector*data-s/s"
 PREC = {"ffma": 0, "f16": 1, "split": 2}
-PREC_DTYPE = {"ffma": "f32", "f16": "f16 operands, f32 accumulate", "split": "f16 hi+lo split operands (3 MMAs), f32 accumulate"}
+PREC_DTYPE = {"ffma": "f32", "f16": "f16 operands, f32 accumulate", "split": "f16 product + fp8 (e4m3 x e5m2) hi/lo correction MMA, f32 accumulate"}
 HEADLINE_CONFIG = 5                  # BASELINE.json configs[4]: the largest single-GPU workload
 NESTED_CONFIGS = (2, 3, 4)           # carried inside the headline line
 

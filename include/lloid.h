@@ -42,7 +42,8 @@ typedef enum {
 typedef enum {
   LLOID_PREC_FP32_FFMA = 0, /* every contraction in fp32 on the CUDA cores (gate 1e-4 of SNR rms)              */
   LLOID_PREC_F16 = 1,       /* tcgen05 kind::f16, operands rounded once to fp16, fp32 accumulate in TMEM         */
-  LLOID_PREC_F16_SPLIT = 2  /* tcgen05 kind::f16, every operand split hi+lo fp16, 3 MMAs per product (default)  */
+  LLOID_PREC_F16_SPLIT = 2  /* default (gate 2e-3, measured 2e-4): fp16 main product + one fp8 (e4m3 x e5m2) MMA that
+                               carries both hi/lo cross terms a_hi b_lo + a_lo b_hi: 2 MMAs per product            */
 } lloid_precision;
 
 /* One time slice of an SVD bank.  Arrays may be host or device memory; create copies them. */
