@@ -129,6 +129,19 @@ int lloid_stream_push(lloid_stream *stream, const float *strain, lloid_peak *pea
  * Errors: EINVAL (null pointer, more than LLOID_MAX_DET detectors, negative window), ECUDA. */
 int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int32_t *dt_samples, lloid_event *events);
 
+/* xi^2 in the stream (Eq. 10).  lloid_bank_set_autocorrelation attaches the bank's template
+ * autocorrelations (before lloid_stream_create): acorr [n_templates][2*delta+1][2] fp32 (re, im), host or device, R_j(t) for
+ * t = -delta..delta with R_j(0) = 1 (definition below).  When EVERY bank of a stream carries autocorrelations of one delta
+ * (and the stream is LLOID_PREC_F16_SPLIT with buffer_len a multiple of 128 and > delta) every push also keeps its
+ * upsampled basis outputs in a three-buffer history ring, and lloid_stream_xi2 evaluates Eq. 10 for the triggers of the push
+ * BEFORE the last one (their windows reach delta samples into the last push: the padding / latency of Fig. 5) with a second
+ * reconstruction pass over [-delta, buffer_len + delta) whose epilogue accumulates |z - z(0) R_j|^2 over each template's own
+ * window; the SNR is still never written to HBM.
+ *   xi2_out  DEVICE, [n_detectors][sum_b M_b] fp32, aligned with the peaks of that push; -1 where it reported no trigger.
+ * Samples before the start of the stream count as zero.  Errors: EINVAL, ESTATE (not enabled / fewer than two pushes), ECUDA. */
+int lloid_bank_set_autocorrelation(lloid_bank *bank, const float *acorr, int32_t delta);
+int lloid_stream_xi2(lloid_stream *stream, float *xi2_out);
+
 /* Signal-based consistency statistic xi^2 of Eq. 10 for the triggers of ONE bank whose SNR series is
  * materialised in device memory (the snr_debug output of lloid_stream_push; the caller keeps consecutive buffers side by
  * side so that the +-delta samples around a trigger are present -- the padding of Fig. 5 -- and calls this one buffer

@@ -62,6 +62,8 @@ def _load():
         "lloid_whitener_hop_in": (i32, [vp]),
         "lloid_whitener_hop_out": (i32, [vp]),
         "lloid_whitener_psd_bins": (i32, [vp]),
+        "lloid_bank_set_autocorrelation": (C.c_int, [vp, vp, i32]),
+        "lloid_stream_xi2": (C.c_int, [vp, vp]),
         "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
@@ -82,7 +84,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
            "lloid_whitener_destroy", "lloid_whitener_hop_in", "lloid_whitener_hop_out", "lloid_whitener_psd_bins", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
@@ -265,7 +267,7 @@ class LloidStream:
 
     def __init__(self, banks, n_detectors: int, buffer_len: int, precision: int = LLOID_PREC_F16_SPLIT,
                  threshold: float = 0.0, device: str = "cuda:0", n_down: int = 32, bank_handles=None, Ms=None,
-                 trigger_overlap: int = 0):
+                 trigger_overlap: int = 0, acorr=None):
         """banks: iterable of Bank-like objects (uploaded here, owned by this object), or None with `bank_handles`
         (+ their template counts `Ms`): existing lloid_bank handles owned by the caller (several streams can share them)."""
         import torch
@@ -283,6 +285,10 @@ class LloidStream:
             for b in banks:                  # any iterable: a generator lets the caller build banks one at a time
                 self.Ms.append(b.M)
                 self.bank_handles.append(lloid_bank_create(b.f0, b.M, bank_slices(b), precision, threshold, n_down, trigger_overlap))
+                if acorr is not None:       # list of complex [M][2 delta + 1] arrays, one per bank (xi^2 of Eq. 10)
+                    a = np.asarray(acorr[len(self.bank_handles) - 1])
+                    a32 = np.ascontiguousarray(np.stack([a.real, a.imag], axis=-1), dtype=np.float32)
+                    _check(_lib.lloid_bank_set_autocorrelation(self.bank_handles[-1], a32.ctypes.data, (a.shape[1] - 1) // 2))
         self.cuda_stream = torch.cuda.current_stream(self.device)
         self.handle = lloid_stream_create(self.bank_handles, n_detectors, buffer_len, self.cuda_stream.cuda_stream)
         self.Mtot = lloid_stream_total_templates(self.handle)
@@ -310,6 +316,14 @@ class LloidStream:
         t.cuda.synchronize(self.device)
         peaks = self.peaks_dev.cpu().numpy().view(PEAK_DTYPE).reshape(self.n_det, self.Mtot)
         return (peaks, snr.cpu().numpy()) if snr is not None else peaks
+
+    def xi2(self):
+        """xi^2 of the triggers of the push before the last one: float32 [n_det][Mtot] (-1 = no trigger)."""
+        t = self.torch
+        out = t.empty((self.n_det, self.Mtot), dtype=t.float32, device=self.device)
+        _check(_lib.lloid_stream_xi2(self.handle, out.data_ptr()))
+        t.cuda.synchronize(self.device)
+        return out.cpu().numpy()
 
     def events(self, dt_samples, peaks_dev=None):
         """Coincidence + clustering on the peaks of the last push (device): structured array [n_banks] (EVENT_DTYPE)."""

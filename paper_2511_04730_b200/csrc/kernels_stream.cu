@@ -426,6 +426,32 @@ __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_d
   peaks[t] = o;
 }
 
+// xi^2 support: copy this push's upsampled Y into slot `slot` of the three-buffer history ring (16-byte vectors)
+__global__ void yup_copy_kernel(const YupCopy *__restrict__ table, int slot) {
+  const YupCopy c = table[blockIdx.y];
+  uint4 *dst = c.dst + (long long)slot * c.dst_slot_stride16;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < c.n16; i += (long long)gridDim.x * blockDim.x) dst[i] = c.src[i];
+}
+cudaError_t launch_yup_copy(const YupCopy *table_dev, int n_pieces, int slot, cudaStream_t st) {
+  if (n_pieces == 0) return cudaSuccess;
+  yup_copy_kernel<<<dim3(8, n_pieces), 256, 0, st>>>(table_dev, slot);
+  return cudaGetLastError();
+}
+// xi^2 = sum of the four column-slice partial numerators (fixed order) / sum_t (2 - 2 |R|^2); -1 where there is no trigger
+__global__ void xi2_finalize_kernel(const float *__restrict__ part, const lloid_peak *__restrict__ peaks, const float *__restrict__ den,
+                                    long long n, int Mtot, float *__restrict__ out) {
+  const long long t = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= n) return;
+  const float4 p = reinterpret_cast<const float4 *>(part)[t];
+  out[t] = peaks[t].sample == LLOID_NO_TRIGGER ? -1.f : (((p.x + p.y) + p.z) + p.w) / den[t % Mtot];
+}
+cudaError_t launch_xi2_finalize(const float *xi_partial, const lloid_peak *peaks, const float *den, int n_det, int Mtot, float *xi2_out,
+                                cudaStream_t st) {
+  const long long n = (long long)n_det * Mtot;
+  xi2_finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(xi_partial, peaks, den, n, Mtot, xi2_out);
+  return cudaGetLastError();
+}
+
 __global__ void fill_partial_kernel(PeakPartial *partial, size_t n) {
   const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) { PeakPartial e; e.p = -3.f; e.idx = 0x7fffffff; e.re = 0.f; e.im = 0.f; partial[i] = e; }

@@ -42,11 +42,17 @@ struct TcReconBank {                         // device copy, 64-byte aligned (CU
   CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle (resident variant)
   CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
   CUtensorMap mapR64, mapY64;                // the same arrays, box 64 x 128, 128-byte swizzle (streaming variant)
+  CUtensorMap mapYh;                         // xi^2: [planes*n_det*3B rows][Kpad] history ring of upsampled Y, box 64 x 128
+  const float2 *acorr;                       // xi^2: [M][2 xi_delta + 1] autocorrelations
   int M, Mpad, Kpad, tmpl_off;
   float inv_scale;
-  int pad_[11];
+  int xi_delta;
+  int pad_[8];
 };
 static_assert(sizeof(TcReconBank) % 64 == 0, "CUtensorMap members need 64-byte alignment");
+struct XiArgs {                              // xi^2 pass (template XI): triggers of the target buffer, output, ring position
+  const lloid_peak *peaks; float *partial; int row_base, ring_rows;
+};
 struct TcCorrClass {
   CUtensorMap mapU;                          // [planes*Lpad rows][Npad] fp16, box 64 x 128
   int pad_[32];
@@ -61,12 +67,12 @@ struct TcCorrClass {
 // RES_KMAX), all K blocks of the item's R tile are loaded ONCE into a resident shared-memory region; only the
 // upsampled-Y blocks stream through the ring.  The streaming variant (any Kpad) moves R and Y blocks together.
 // ------------------------------------------------------------------------------------------------
-template <int PLANES, bool RES>
+template <int PLANES, bool RES, bool XI = false>
 __global__ void __launch_bounds__(RECON_THREADS, 1)
 recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__restrict__ tiles, const int *__restrict__ cta_begin,
                 int n_det, int B,
                 PeakPartial *__restrict__ partial, int Mtot, int n_tt, float *__restrict__ snr_debug, int debug_bank,
-                int ring_off, int n_stages, int t_min) {
+                int ring_off, int n_stages, int t_min, XiArgs xi = XiArgs()) {
   constexpr int RBK = RES ? RBK_RES : RBK_STR;
   constexpr int RTILE_BYTES = TILE_M * RBK * 2;
   // Operand ring of K blocks of RBK (tiles of 128 rows x RBK fp16).  Streaming: NT = 3 * PLANES tiles
@@ -114,7 +120,15 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         }
         for (int d = 0; d < tl.ndet; ++d)
         for (int tt = 0; tt < tl.nt; ++tt) {
-          const int yrow = (tl.det + d) * B + tl.t0 + tt * TILE_N;
+          int yrow = (tl.det + d) * B + tl.t0 + tt * TILE_N;
+          int yplane = n_det * B;                                  // rows between the planes of the Y array
+          if (XI) {
+            // history ring: sample t of the target buffer sits at row (row_base + t) mod ring_rows (t may be negative)
+            int r = (xi.row_base + tl.t0 + tt * TILE_N) % xi.ring_rows;
+            if (r < 0) r += xi.ring_rows;
+            yrow = (tl.det + d) * xi.ring_rows + r;
+            yplane = n_det * xi.ring_rows;
+          }
           for (int kb = 0; kb < nkb; ++kb) {
             mbar_wait(&empty[stage], phase ^ 1);
             mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
@@ -127,7 +141,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
               for (int p = 0; p < PLANES; ++p) {
                 tma_load_2d(sdst + (3 * p + 0) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 0) * bk->Mpad + tl.m0);
                 tma_load_2d(sdst + (3 * p + 1) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 1) * bk->Mpad + tl.m0);
-                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, &bk->mapY64, &full[stage], kb * RBK, p * n_det * B + yrow);
+                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, XI ? &bk->mapYh : &bk->mapY64, &full[stage], kb * RBK, p * yplane + yrow);
               }
             }
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
@@ -208,6 +222,47 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       const TcReconBank *bk = &banks[tl.bank];
       const int m = tl.m0 + q * 32 + lane, M = bk->M, tmpl_off = bk->tmpl_off;
       const float sc = bk->inv_scale;
+      if (XI) {
+        // xi^2 pass (Eq. 10): the item covers samples [t0, t0 + 128 nt) around the target buffer; this
+        // thread accumulates |z[t] - z0 R_j[t - k0]|^2 over the window of ITS template's trigger (raw accumulator scale)
+        const int det = tl.det, delta = bk->xi_delta;
+        lloid_peak pk; pk.snr = 0.f; pk.sample = LLOID_NO_TRIGGER; pk.phase = 0.f;
+        if (m < M) pk = xi.peaks[(size_t)det * Mtot + tmpl_off + m];
+        const bool has = pk.sample != LLOID_NO_TRIGGER;
+        const int k0 = has ? pk.sample : 0;
+        float sn, cs_;
+        sincosf(pk.phase, &sn, &cs_);
+        const float z0r = pk.snr * cs_ / sc, z0i = pk.snr * sn / sc;
+        const float2 *R = bk->acorr + (size_t)(m < M ? m : 0) * (2 * delta + 1);
+        float num = 0.f;
+        for (int tt = 0; tt < tl.nt; ++tt, ++it) {
+          const int buf = it & 1;
+          const int tbase = tl.t0 + tt * TILE_N + cs * 32;
+          mbar_wait(&tfull[buf], (it >> 1) & 1);
+          tc_fence_after_sync();
+          const uint32_t t_re = tmem + lane_base + buf * 256 + cs * 32;
+          uint32_t vr[32], vi[32];
+          tmem_ld_32x32(t_re, vr);
+          tmem_ld_32x32(t_re + 128, vi);
+          tmem_ld_wait();
+          tc_fence_before_sync();
+          __syncwarp();
+          if (lane == 0) mbar_arrive(&tempty[buf]);
+          if (has && tbase + 31 >= k0 - delta && tbase <= k0 + delta) {
+#pragma unroll
+            for (int i = 0; i < 32; ++i) {
+              const int u = tbase + i - k0 + delta;
+              if (u >= 0 && u <= 2 * delta) {
+                const float2 a = R[u];
+                const float dr = __uint_as_float(vr[i]) - (z0r * a.x - z0i * a.y), di = __uint_as_float(vi[i]) - (z0r * a.y + z0i * a.x);
+                num = fmaf(dr, dr, fmaf(di, di, num));
+              }
+            }
+          }
+        }
+        if (m < M) xi.partial[((size_t)det * Mtot + tmpl_off + m) * 4 + cs] = num * sc * sc;
+        continue;
+      }
       const bool dbg = snr_debug != nullptr && tl.bank == debug_bank && m < M;
       for (int d = 0; d < tl.ndet; ++d) {
       const int det = tl.det + d;
@@ -565,6 +620,7 @@ struct TcPlan {
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
   TcReconTile *res_items_dev; int *res_begin_dev; int n_res_items, res_grid, res_ring_off, res_stages, str_stages;   // resident-R a3
   TcReconTile *tail_dev; int *tail_begin_dev; int n_tail, tail_grid, tail_tmin;   // tail pass of overlapped trigger windows
+  TcReconTile *xi_dev; int *xi_begin_dev; int n_xi, xi_grid;   // xi^2 pass
   int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
   const CorrClass *classes_dev;
@@ -667,7 +723,7 @@ void tc_plan_destroy(TcPlan *p) {
 }
 
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
-                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes, int overlap) {
+                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes, int overlap, int xi_delta) {
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
@@ -731,6 +787,8 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
         !make_map(&rb[b].mapR64, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_STR) ||
         !make_map(&rb[b].mapY64, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
+    rb[b].acorr = k.acorr; rb[b].xi_delta = k.xi_delta;
+    if (xi_delta > 0 && !make_map(&rb[b].mapYh, k.yhist, (uint64_t)planes * n_det * 3 * B, (uint64_t)k.Kpad, TILE_M, RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
     // resident R pays when the item reuses it over enough tiles (short buffers, config 4, stream R with Y instead)
     is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && (long long)n_det * ((B + TILE_N - 1) / TILE_N) >= 8) ? 1 : 0;
     const long long mt = (k.M + TILE_M - 1) / TILE_M;
@@ -769,6 +827,16 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
       for (int m0 = 0; m0 < banks[b].M; m0 += TILE_M)
         for (int det = 0; det < n_det; ++det) tail.push_back({(int)b, det, 1, m0, i0 * TILE_N, ntile - i0, 0});
   }
+  // xi^2 pass: per (bank, template tile, detector) the 128-aligned tiles covering [-delta, B + delta) of the target buffer
+  std::vector<TcReconTile> xit;
+  if (xi_delta > 0) {
+    const int t_first = -((xi_delta + TILE_N - 1) / TILE_N) * TILE_N, nt_xi = (B + xi_delta - t_first + TILE_N - 1) / TILE_N;
+    for (size_t b = 0; b < banks.size(); ++b)
+      for (int m0 = 0; m0 < banks[b].M; m0 += TILE_M)
+        for (int det = 0; det < n_det; ++det) xit.push_back({(int)b, det, 1, m0, t_first, nt_xi, 0});
+  }
+  p->n_xi = (int)xit.size();
+  p->xi_grid = std::max(1, std::min(p->n_xi, sms));
   p->n_tail = (int)tail.size();
   p->tail_grid = std::max(1, std::min(p->n_tail, sms));
   p->n_res_items = (int)ri.size();
@@ -787,10 +855,12 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   lpt_assign(ri, p->res_grid, [&](const TcReconTile &t) {
     const long long kp = rb[t.bank].Kpad;
     return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 388, 600) + 3000 + kp * 8; }, ibegin);
-  std::vector<int> tbegin;
+  std::vector<int> tbegin, xbegin;
+  lpt_assign(xit, p->xi_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, xbegin);
   lpt_assign(tail, p->tail_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, tbegin);
   if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->res_items_dev, ri) ||
-      !plan_upload(p, &p->res_begin_dev, ibegin) || !plan_upload(p, &p->tail_dev, tail) || !plan_upload(p, &p->tail_begin_dev, tbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+      !plan_upload(p, &p->res_begin_dev, ibegin) || !plan_upload(p, &p->tail_dev, tail) || !plan_upload(p, &p->tail_begin_dev, tbegin) ||
+      !plan_upload(p, &p->xi_dev, xit) || !plan_upload(p, &p->xi_begin_dev, xbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   p->recon_smem = RECON_SMEM_BUDGET + 1024 + 256;
@@ -799,6 +869,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   if (planes == 2) {
     e = cudaFuncSetAttribute(recon_tc_kernel<2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(recon_tc_kernel<2, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
+    if (e == cudaSuccess) e = cudaFuncSetAttribute(recon_tc_kernel<2, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
     if (e == cudaSuccess) e = cudaFuncSetAttribute(corr_tc_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->corr_smem);
   } else {
     e = cudaFuncSetAttribute(recon_tc_kernel<1, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, p->recon_smem);
@@ -820,6 +891,14 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
 
 int tc_plan_n_tt(const TcPlan *p) { return p->n_tt; }
 int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_res_items ? 1 : 0) + (p->n_tail ? 1 : 0); }
+
+cudaError_t tc_launch_xi2(TcPlan *p, const lloid_peak *peaks, float *xi_partial, int Mtot, int row_base, cudaStream_t st) {
+  if (p->n_xi == 0 || p->planes != 2) return cudaErrorInvalidValue;
+  XiArgs xa; xa.peaks = peaks; xa.partial = xi_partial; xa.row_base = row_base; xa.ring_rows = 3 * p->B;
+  recon_tc_kernel<2, false, true><<<p->xi_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->xi_dev, p->xi_begin_dev, p->n_det, p->B,
+                                                                                  nullptr, Mtot, 4, nullptr, -1, 0, p->str_stages, 0, xa);
+  return cudaGetLastError();
+}
 
 // tail pass: the peak of every template over the buffer's last `overlap` samples -> tail_partial [n_det][Mtot][4]
 cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st) {

@@ -41,6 +41,8 @@ extern "C" void lloid_bank_destroy(lloid_bank *b) {
   if (!b) return;
   if (b->dR32) cudaFree(b->dR32);
   if (b->dR16) cudaFree(b->dR16);
+  if (b->dAcorr) cudaFree(b->dAcorr);
+  if (b->dXiDen) cudaFree(b->dXiDen);
   delete b;
 }
 
@@ -88,6 +90,7 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
   if (!b) { set_error("bank_create: out of host memory"); return LLOID_ENOMEM; }
   b->f0 = f0; b->M = M; b->Mpad = (M + 127) / 128 * 128; b->S = S; b->opt = opt;
   b->dR32 = nullptr; b->dR16 = nullptr; b->r_scale = 1.f; b->r_planes = 0;
+  b->dAcorr = nullptr; b->dXiDen = nullptr; b->xi_delta = 0;
   // ---- groups = runs of equal rate; halo recursion of the zero-phase chain (oracle: upsample_input_range)
   int koff = 0;
   for (int s = 0; s < S; ++s) {
@@ -186,5 +189,33 @@ extern "C" int lloid_bank_create(lloid_bank **out, int32_t f0, int32_t M, int32_
   }
   if (e != cudaSuccess) { set_error("bank_create: upload of R failed: %s", cudaGetErrorString(e)); lloid_bank_destroy(b); return LLOID_ECUDA; }
   *out = b;
+  return LLOID_OK;
+}
+
+// Template autocorrelations for the xi^2 statistic of Eq. 10: R_j(t), t = -delta..delta.
+extern "C" int lloid_bank_set_autocorrelation(lloid_bank *b, const float *acorr, int32_t delta) {
+  if (!b || !acorr || delta < 1) { set_error("bank_set_autocorrelation: NULL pointer or delta < 1"); return LLOID_EINVAL; }
+  const size_t n = (size_t)b->M * (2 * (size_t)delta + 1);
+  std::vector<float> h(2 * n);
+  cudaError_t e = cudaMemcpy(h.data(), acorr, h.size() * sizeof(float), cudaMemcpyDefault);
+  if (e != cudaSuccess) { set_error("bank_set_autocorrelation: copy failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  std::vector<float> den(b->M);
+  for (int j = 0; j < b->M; ++j) {
+    double d = 0;
+    for (int u = 0; u <= 2 * delta; ++u) {
+      const double re = h[2 * ((size_t)j * (2 * delta + 1) + u)], im = h[2 * ((size_t)j * (2 * delta + 1) + u) + 1];
+      d += 2.0 - 2.0 * (re * re + im * im);
+    }
+    den[j] = (float)d;
+  }
+  if (b->dAcorr) { cudaFree(b->dAcorr); b->dAcorr = nullptr; }
+  if (b->dXiDen) { cudaFree(b->dXiDen); b->dXiDen = nullptr; }
+  if (cudaMalloc(&b->dAcorr, n * sizeof(float2)) != cudaSuccess || cudaMalloc(&b->dXiDen, b->M * sizeof(float)) != cudaSuccess) {
+    set_error("bank_set_autocorrelation: cudaMalloc failed"); return LLOID_ENOMEM;
+  }
+  e = cudaMemcpy(b->dAcorr, h.data(), n * sizeof(float2), cudaMemcpyHostToDevice);
+  if (e == cudaSuccess) e = cudaMemcpy(b->dXiDen, den.data(), b->M * sizeof(float), cudaMemcpyHostToDevice);
+  if (e != cudaSuccess) { set_error("bank_set_autocorrelation: upload failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  b->xi_delta = delta;
   return LLOID_OK;
 }

@@ -43,6 +43,9 @@ struct lloid_bank {
   float *dR32;                       // FFMA:   [2 (re,im)][Mpad][Kpad] fp32
   __half *dR16;                      // tensor: [planes (hi,lo)][2 (re,im)][Mpad][Kpad] fp16, scaled by r_scale
   int r_planes;
+  float2 *dAcorr;                    // [M][2 xi_delta + 1] template autocorrelations R_j(t) (Eq. 10), nullptr = none
+  float *dXiDen;                     // [M] sum_t (2 - 2 |R_j(t)|^2)
+  int xi_delta;
 };
 
 // ---------------------------------------------------------------------------------------------- device tables
@@ -98,6 +101,8 @@ struct ReconBank {                   // a3 work description of one bank
   const float *R32; const __half *R16; long long r_part_stride, r_plane_stride;
   const void *yup; long long yup_det_stride, yup_plane_stride;
   int M, Mpad, Kpad, tmpl_off;       // tmpl_off: first template of this bank in the stream's peak array
+  const void *yhist;                 // xi^2: [planes][n_det][3 B][Kpad] ring of the last three pushes' upsampled Y (or nullptr)
+  const float2 *acorr; int xi_delta; // xi^2: the bank's autocorrelations
   float inv_scale2;                  // 1/(r_scale^2): applied to |z|^2
   float inv_scale;
 };
@@ -114,6 +119,10 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
                             const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st);
 cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
+struct YupCopy { const uint4 *src; uint4 *dst; long long n16; long long dst_slot_stride16; };   // one (bank, plane, detector) piece
+cudaError_t launch_yup_copy(const YupCopy *table_dev, int n_pieces, int slot, cudaStream_t st);
+cudaError_t launch_xi2_finalize(const float *xi_partial, const lloid_peak *peaks, const float *den, int n_det, int Mtot, float *xi2_out,
+                                cudaStream_t st);
 cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st);
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
                             lloid_peak *peaks, long long *n0, int B, PeakPartial *tail, const PeakPartial *tail_partial, int overlap,
@@ -127,7 +136,8 @@ struct TcPlan;
 int tc_time_splits(int B, long long n_mtile_units);   // n_mtile_units = sum_banks ceil(M/128) * n_det
 int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel for a slice of Npad taps   // partial peaks per template written by the tensor-core a3 kernel
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
-                   const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes, int overlap);
+                   const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes, int overlap,
+                   int xi_delta);
 void tc_plan_destroy(TcPlan *p);
 int tc_plan_n_tt(const TcPlan *p);              // partial peaks per template and detector the a3 kernels write
 int tc_plan_recon_launches(const TcPlan *p);    // 1 or 2: streaming kernel and / or resident-R kernel
@@ -135,5 +145,7 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st);
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank,
                             cudaStream_t st);
 cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st);
+// xi^2 pass over [-delta, B + delta) of the buffer whose upsampled Y sits at ring rows [row_base, row_base + B) (mod 3 B)
+cudaError_t tc_launch_xi2(TcPlan *p, const lloid_peak *peaks, float *xi_partial, int Mtot, int row_base, cudaStream_t st);
 
 }  // namespace lloid

@@ -18,6 +18,11 @@ struct lloid_stream {
   std::vector<const lloid_bank *> banks;
   int n_det, B, f0, precision, n_down, Mtot, n_tt, max_mtiles, overlap;
   int *bank_off_dev;                               // [n_banks + 1] template offsets (coincidence / clustering)
+  int xi_delta;                                    // > 0: xi^2 enabled (every bank carries autocorrelations of this half width)
+  YupCopy *ycopy_dev; int n_ycopy;                 // xi^2: pieces of the per-push copy of upsampled Y into the history ring
+  lloid_peak *peaks_hist[2];                       // xi^2: triggers of the last two pushes
+  float *xi_partial_dev, *xi_den_dev;              // xi^2: [n_det][Mtot][4] numerators; [Mtot] denominators
+  long long n_pushes;
   PeakPartial *tail_dev, *tail_partial_dev;        // overlapped trigger windows: previous buffer's tail peak, this buffer's partials
   float threshold;
   cudaStream_t st;
@@ -115,6 +120,13 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->n_det = n_det; s->B = B; s->f0 = banks[0]->f0; s->precision = banks[0]->opt.precision;
   s->n_down = banks[0]->opt.n_down; s->threshold = banks[0]->opt.threshold; s->overlap = banks[0]->opt.trigger_overlap;
   s->tail_dev = nullptr; s->tail_partial_dev = nullptr;
+  s->n_pushes = 0; s->n_ycopy = 0; s->ycopy_dev = nullptr; s->peaks_hist[0] = s->peaks_hist[1] = nullptr;
+  s->xi_partial_dev = s->xi_den_dev = nullptr;
+  // xi^2 (Eq. 10) runs when EVERY bank carries autocorrelations of one half width; it needs the split tensor mode and
+  // 128-sample-aligned buffers longer than the half width (the history ring is addressed in whole tiles)
+  s->xi_delta = banks[0]->xi_delta;
+  for (int b = 0; b < n_banks; ++b) if (banks[b]->xi_delta != s->xi_delta) s->xi_delta = 0;
+  if (s->precision != LLOID_PREC_F16_SPLIT || B % 128 != 0 || s->xi_delta >= B) s->xi_delta = 0;
   s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false; s->failed = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
@@ -273,6 +285,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   // rows are grouped by upsample chain (stage factors) so that a warp's 32 lanes are 32 rows of ANY slices / banks
   // sharing the chain; within a chain they are ordered by (bank, column) to keep the stores contiguous
   std::map<std::vector<int>, std::vector<UpRow>> chains;
+  std::vector<YupCopy> ycopies;
   s->Mtot = 0; s->max_mtiles = 0;
   for (int b = 0; b < n_banks; ++b) {
     const lloid_bank *bk = s->banks[b];
@@ -281,6 +294,17 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     void *yup = nullptr;
     if (s->up_planes == 0) { float *p; CK(dev_alloc(s, &p, plane_elems)); yup = p; }
     else { __half *p; CK(dev_alloc(s, &p, plane_elems * planes)); yup = p; }
+    if (s->xi_delta > 0) {
+      __half *h; CK(dev_alloc(s, &h, plane_elems * planes * 3, true));        // zero = "before the stream started"
+      rb.yhist = h; rb.acorr = bk->dAcorr; rb.xi_delta = bk->xi_delta;
+      for (int pd = 0; pd < planes * n_det; ++pd) {
+        YupCopy c;
+        c.src = reinterpret_cast<const uint4 *>((const __half *)yup + (size_t)pd * B * bk->Kpad);
+        c.dst = reinterpret_cast<uint4 *>(h + (size_t)pd * 3 * B * bk->Kpad);
+        c.n16 = (long long)B * bk->Kpad * 2 / 16; c.dst_slot_stride16 = c.n16;
+        ycopies.push_back(c);
+      }
+    }
     rb.R32 = bk->dR32; rb.R16 = bk->dR16;
     rb.r_part_stride = (long long)bk->Mpad * bk->Kpad; rb.r_plane_stride = 2 * rb.r_part_stride;
     rb.yup = yup; rb.yup_det_stride = (long long)B * bk->Kpad; rb.yup_plane_stride = (long long)plane_elems;
@@ -349,7 +373,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
   if (s->precision != LLOID_PREC_FP32_FFMA) {
-    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap);
+    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap, s->xi_delta);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
     s->n_tt = tc_plan_n_tt(s->tc);                 // partial peaks per template: the larger of the two a3 kernels' splits
     s->work[0] *= (planes == 2 ? 2 : 1);           // split mode: two MMAs per product in a2 (U_hi x, U_lo x) and in a3
@@ -363,6 +387,16 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     CK(dev_alloc(s, &s->tail_dev, (size_t)n_det * s->Mtot, true));
     CK(dev_alloc(s, &s->tail_partial_dev, (size_t)n_det * s->Mtot * 4));
     CK(launch_fill_partial(s->tail_partial_dev, (size_t)n_det * s->Mtot * 4, s->st));
+  }
+  if (s->xi_delta > 0) {
+    s->n_ycopy = (int)ycopies.size();
+    CK(dev_upload(s, &s->ycopy_dev, ycopies));
+    CK(dev_alloc(s, &s->peaks_hist[0], (size_t)n_det * s->Mtot));
+    CK(dev_alloc(s, &s->peaks_hist[1], (size_t)n_det * s->Mtot));
+    CK(dev_alloc(s, &s->xi_partial_dev, (size_t)n_det * s->Mtot * 4));
+    CK(dev_alloc(s, &s->xi_den_dev, (size_t)s->Mtot));
+    for (size_t b = 0; b < s->banks.size(); ++b)
+      CK(cudaMemcpy(s->xi_den_dev + s->rbanks[b].tmpl_off, s->banks[b]->dXiDen, sizeof(float) * s->banks[b]->M, cudaMemcpyDeviceToDevice));
   }
   CK(cudaDeviceSynchronize());
   *out = s;
@@ -399,6 +433,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   if (e == cudaSuccess)
     e = launch_upsample(s->items_dev, s->uprows_dev, s->n_items, s->n_det, s->B, s->up_chunk, s->uptaps_dev, s->uptap_off_dev,
                         s->n0_dev, s->up_planes, s->taps2, s->st);
+  if (e == cudaSuccess && s->xi_delta > 0) e = launch_yup_copy(s->ycopy_dev, s->n_ycopy, (int)(s->n_pushes % 3), s->st);
   mark(3);
   if (e == cudaSuccess) {
     where = "a3 reconstruct";
@@ -412,6 +447,8 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   if (e == cudaSuccess)
     e = launch_finalize(s->partial_dev, s->n_det, s->Mtot, s->n_tt, s->threshold, peaks, s->n0_dev, s->B, s->tail_dev,
                         s->tail_partial_dev, s->overlap, s->st);
+  if (e == cudaSuccess && s->xi_delta > 0)
+    e = cudaMemcpyAsync(s->peaks_hist[s->n_pushes & 1], peaks, sizeof(lloid_peak) * s->n_det * s->Mtot, cudaMemcpyDeviceToDevice, s->st);
   mark(5);
   if (s->stage_timing) s->ev_rec.push_back(std::move(ev));
   if (e != cudaSuccess) {
@@ -421,6 +458,20 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
     set_error("stream_push: launch of %s failed: %s (stream needs lloid_state_reset)", where, cudaGetErrorString(e)); return LLOID_ECUDA;
   }
   s->n0_host += s->B;
+  s->n_pushes += 1;
+  return LLOID_OK;
+}
+
+// xi^2 (Eq. 10) of the triggers of the push BEFORE the last one: their +-delta windows reach into the last push.
+extern "C" int lloid_stream_xi2(lloid_stream *s, float *xi2_out) {
+  if (!s || !xi2_out) { set_error("stream_xi2: NULL argument"); return LLOID_EINVAL; }
+  if (s->xi_delta <= 0) { set_error("stream_xi2: not enabled (every bank needs lloid_bank_set_autocorrelation with one half width, "
+                                    "LLOID_PREC_F16_SPLIT, buffer_len a multiple of 128 and longer than the half width)"); return LLOID_ESTATE; }
+  if (s->failed || s->n_pushes < 2) { set_error("stream_xi2: needs two pushes (the statistic lags by one buffer)"); return LLOID_ESTATE; }
+  const long long b = s->n_pushes - 2;                              // the target buffer
+  cudaError_t e = tc_launch_xi2(s->tc, s->peaks_hist[b & 1], s->xi_partial_dev, s->Mtot, (int)(b % 3) * s->B, s->st);
+  if (e == cudaSuccess) e = launch_xi2_finalize(s->xi_partial_dev, s->peaks_hist[b & 1], s->xi_den_dev, s->n_det, s->Mtot, xi2_out, s->st);
+  if (e != cudaSuccess) { set_error("stream_xi2: launch failed: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   return LLOID_OK;
 }
 
@@ -456,6 +507,7 @@ extern "C" int lloid_state_reset(lloid_stream *s) {
     if (e != cudaSuccess) { set_error("state_reset: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   }
   s->n0_host = 0;
+  s->n_pushes = 0;
   s->failed = false;
   return LLOID_OK;
 }

@@ -197,3 +197,60 @@ def test_xi2_from_the_materialised_snr_against_the_oracle():
     assert pks[18]["snr"][7] > 11 and 0.3 < got18[7] < 2.5
     none = torch.full((bank.M,), NO_TRIGGER, dtype=torch.int32, device="cuda")
     assert (lib.binding.lloid_xi2_series(snr_all, none, ac_dev, delta).cpu().numpy() == -1).all()
+
+
+@pytest.mark.parametrize("delta", [175, 350])
+def test_xi2_in_the_stream_against_the_oracle(delta):
+    """lloid_stream_xi2: the second reconstruction pass one buffer later (SNR never materialised), 2 detectors x 2 banks,
+    against oracle.xi2 on the float64 LLOID SNR -- for every buffer, including the first (zeros before the stream start)."""
+    _cuda()
+    import paper_2511_04730_b200 as lib
+    from oracle import find_peaks, lloid_snr, xi2
+    from workloads import bank_from_layout, chirp_templates, inject, injection_waveform, make_strain, template_autocorrelations
+    f0, B = 2048, 1024
+    lay = [(2048, 0, 1024), (1024, 1024, 3072), (512, 3072, 8192), (256, 8192, 16384)]
+    mcs = [np.linspace(1.2, 1.4, 21), np.linspace(1.5, 1.8, 150)]           # the second bank has two template tiles
+    banks = [bank_from_layout(mc, 8.0, lay, f0=f0).as_f32() for mc in mcs]
+    acorr = [template_autocorrelations(chirp_templates(mc, 8.0, f0, 1024.0), delta) for mc in mcs]
+    n_push = 20
+    strain = np.stack([make_strain(93 + d, n_push * B) for d in range(2)])
+    inject(strain[1], injection_waveform(float(mcs[1][140]), 8.0, 13.0, 2.1, f0), 17 * B + 1000)   # window crosses a buffer edge
+    st = lib.LloidStream(banks, 2, B, acorr=acorr)
+    with pytest.raises(lib.LloidError):
+        st.xi2()                                                          # needs two pushes
+    pks, xis = [], {}
+    for p in range(n_push):
+        pks.append(st.push(strain[:, p * B:(p + 1) * B]).copy())
+        if p >= 1:
+            xis[p - 1] = st.xi2()
+    st.close()
+    off = [0, 21, 171]
+    worst, n_cmp = 0.0, 0
+    for det in range(2):
+        for b, bank in enumerate(banks):
+            ref = lloid_snr(bank, strain[det])
+            z = ref[0::2] + 1j * ref[1::2]
+            _, idx_o, _ = find_peaks(ref, B)
+            for p in (0, 1, 8, 16, 17, 18):
+                got = xis[p][det, off[b]:off[b + 1]]
+                for j in range(0, bank.M, 3 if bank.M > 50 else 1):
+                    if pks[p]["sample"][det, off[b] + j] != idx_o[p, j]:
+                        continue
+                    want = xi2(z[j], int(idx_o[p, j]) + p * B, acorr[b][j])
+                    worst = max(worst, abs(got[j] - want) / want)
+                    n_cmp += 1
+    print(f"stream xi2 (delta {delta}): {n_cmp} triggers compared, worst relative error {worst:.2e}")
+    assert n_cmp > 250 and worst < 2e-3
+    assert pks[17]["snr"][1, 21 + 140] > 10 and 0.3 < xis[17][1, 21 + 140] < 2.5
+
+
+def test_xi2_is_off_without_autocorrelations():
+    _cuda()
+    import paper_2511_04730_b200 as lib
+    from workloads import make_strain, random_bank
+    st = lib.LloidStream([random_bank(5, 40, [(2048, 256, 8)]).as_f32()], 1, 256)
+    st.push(make_strain(1, 256)[None]); st.push(make_strain(2, 256)[None])
+    with pytest.raises(lib.LloidError) as e:
+        st.xi2()
+    assert e.value.code == lib.binding.LLOID_ESTATE
+    st.close()
