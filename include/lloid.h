@@ -129,6 +129,18 @@ int lloid_stream_push(lloid_stream *stream, const float *strain, lloid_peak *pea
  * Errors: EINVAL (null pointer, more than LLOID_MAX_DET detectors, negative window), ECUDA. */
 int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int32_t *dt_samples, lloid_event *events);
 
+/* SVD bank construction on the GPU (Eq. 3): truncated singular value decomposition of one time slice's
+ * template matrix, the inputs lloid_bank_create takes.  One-sided Jacobi in float64 (own kernels, no library); synchronous.
+ *   H            HOST or DEVICE, [n_rows][n_taps] float64 row-major: the 2M real template rows of the slice
+ *   energy       keep the smallest L with sum_{l<L} sigma_l^2 >= energy * sum sigma^2 (0.9999 in BASELINE.json)
+ *   basis_out    DEVICE, capacity [max_basis][n_taps] fp32: U, L orthonormal rows written compactly as [L][n_taps]
+ *   recon_out    DEVICE, capacity [n_rows][max_basis] fp32: R = V diag(sigma), written compactly as [n_rows][L]
+ *   n_basis_out  HOST: L;  singular_out HOST [max_basis] or NULL: sigma_0 >= sigma_1 >= ...;  kept_energy_out HOST or NULL
+ * H ~= R U with relative residual energy 1 - kept_energy.  Singular vectors are defined up to sign (and up to a rotation
+ * inside a cluster of equal singular values); the product R U is unique.  Errors: EINVAL (sizes, L > max_basis), ENOMEM, ECUDA. */
+int lloid_svd_slice(const double *H, int32_t n_rows, int32_t n_taps, double energy, int32_t max_basis, int32_t *n_basis_out,
+                    float *basis_out, float *recon_out, double *singular_out, double *kept_energy_out, void *cuda_stream);
+
 /* xi^2 in the stream (Eq. 10).  lloid_bank_set_autocorrelation attaches the bank's template
  * autocorrelations (before lloid_stream_create): acorr [n_templates][2*delta+1][2] fp32 (re, im), host or device, R_j(t) for
  * t = -delta..delta with R_j(0) = 1 (definition below).  When EVERY bank of a stream carries autocorrelations of one delta

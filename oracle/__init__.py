@@ -5,3 +5,4 @@ from .lloid_oracle import (  # noqa: F401
 )
 from .events_oracle import find_peaks_overlap, template_acorr, xi2, coincidences, cluster  # noqa: F401,E402
 from .whiten_oracle import Whitener, log_median_mean, hann_periodic, tukey_taper  # noqa: F401,E402
+from .svd_oracle import svd_slice  # noqa: F401,E402

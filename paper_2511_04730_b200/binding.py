@@ -64,6 +64,7 @@ def _load():
         "lloid_whitener_psd_bins": (i32, [vp]),
         "lloid_bank_set_autocorrelation": (C.c_int, [vp, vp, i32]),
         "lloid_stream_xi2": (C.c_int, [vp, vp]),
+        "lloid_svd_slice": (C.c_int, [vp, i32, i32, C.c_double, i32, C.POINTER(i32), vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]),
         "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
@@ -84,7 +85,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_svd_slice", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
            "lloid_whitener_destroy", "lloid_whitener_hop_in", "lloid_whitener_hop_out", "lloid_whitener_psd_bins", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
@@ -173,6 +174,25 @@ def lloid_xi2_series(snr_dev, trigger_sample_dev, acorr_dev, delta: int, cuda_st
     _check(_lib.lloid_xi2_series(snr_dev.data_ptr(), M, n, trigger_sample_dev.data_ptr(), acorr_dev.data_ptr(), delta, out.data_ptr(),
                                  cuda_stream))
     return out
+
+
+def lloid_svd_slice(H: np.ndarray, energy: float = 0.9999, max_basis: Optional[int] = None, device: str = "cuda:0"):
+    """Truncated SVD of a slice's template matrix on the GPU: H float64 [2M][N] (host) -> (U float32 [L][N], R float32 [2M][L],
+    sigma float64 [L], kept energy)."""
+    import torch
+    H = np.ascontiguousarray(H, dtype=np.float64)
+    n, N = H.shape
+    mb = min(n, N) if max_basis is None else max_basis
+    dev = torch.device(device)
+    torch.cuda.set_device(dev)
+    U = torch.empty((mb, N), dtype=torch.float32, device=dev)
+    R = torch.empty((n, mb), dtype=torch.float32, device=dev)
+    L, kept = C.c_int32(), C.c_double()
+    sig = np.zeros(mb)
+    _check(_lib.lloid_svd_slice(H.ctypes.data, n, N, energy, mb, C.byref(L), U.data_ptr(), R.data_ptr(),
+                                sig.ctypes.data_as(C.POINTER(C.c_double)), C.byref(kept), torch.cuda.current_stream(dev).cuda_stream))
+    L = L.value
+    return (U.flatten()[:L * N].reshape(L, N).cpu().numpy(), R.flatten()[:n * L].reshape(n, L).cpu().numpy(), sig[:L].copy(), kept.value)
 
 
 def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):

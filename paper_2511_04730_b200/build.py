@@ -11,7 +11,7 @@ import sys
 
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
-SOURCES = ["lloid_bank.cu", "lloid_stream.cu", "lloid_events.cu", "lloid_whiten.cu", "kernels_stream.cu", "kernels_ffma.cu", "kernels_tc.cu"]
+SOURCES = ["lloid_bank.cu", "lloid_stream.cu", "lloid_events.cu", "lloid_whiten.cu", "lloid_svd.cu", "kernels_stream.cu", "kernels_ffma.cu", "kernels_tc.cu"]
 LIB = os.path.join(HERE, "liblloid.so")
 NVCC = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
 FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", "-Xcompiler", "-fPIC",

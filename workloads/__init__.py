@@ -15,6 +15,7 @@ from .lloid_inputs import (  # noqa: F401
     slice_layout,
     build_bank,
     bank_from_layout,
+    slice_template_matrices,
     decompose_slice,
     injection_waveform,
     random_bank,

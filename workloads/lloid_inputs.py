@@ -209,14 +209,15 @@ def decompose_slice(Hs: np.ndarray, energy: Optional[float] = 0.9999, method: st
     raise ValueError(method)
 
 
-def bank_from_layout(mchirp: Sequence[float], T: float, layout: Sequence[Tuple[int, int, int]],
-                     f0: int = F0_HZ, energy: Optional[float] = 0.9999, f_max: float = 1024.0,
-                     method: str = "svd") -> Bank:
+def slice_template_matrices(mchirp: Sequence[float], T: float, layout: Sequence[Tuple[int, int, int]],
+                            f0: int = F0_HZ, f_max: float = 1024.0) -> List[np.ndarray]:
+    """Per slice the template matrix H^s [2M][N^s] (float64) that the SVD of PAPER.md:112-119 decomposes: the analytic chirps
+    evaluated on the slice's coarse grid, oldest tap first, rows scaled by sqrt(D) / (full-rate norm)."""
     mchirp = np.asarray(mchirp, dtype=np.float64)
     M = len(mchirp)
     N = int(round(T * f0))
     norms = [_chirp_norms(mc, N, f0, f_max) for mc in mchirp]
-    slices = []
+    out = []
     for rate, Bs, Es in layout:
         D = f0 // rate
         assert Bs % D == 0 and Es % D == 0 and Es > Bs
@@ -228,9 +229,20 @@ def bank_from_layout(mchirp: Sequence[float], T: float, layout: Sequence[Tuple[i
             c, s = _chirp_quadratures(mc, a, N, f0, f_max)
             Hs[2 * j] = c * (math.sqrt(D) / norms[j][0])
             Hs[2 * j + 1] = s * (math.sqrt(D) / norms[j][1])
+        out.append(Hs)
+    return out
+
+
+def bank_from_layout(mchirp: Sequence[float], T: float, layout: Sequence[Tuple[int, int, int]],
+                     f0: int = F0_HZ, energy: Optional[float] = 0.9999, f_max: float = 1024.0,
+                     method: str = "svd") -> Bank:
+    mchirp = np.asarray(mchirp, dtype=np.float64)
+    slices = []
+    for (rate, Bs, Es), Hs in zip(layout, slice_template_matrices(mchirp, T, layout, f0, f_max)):
+        D = f0 // rate
         U, R, kept = decompose_slice(Hs, energy, method)
-        slices.append(Slice(rate=rate, n_taps=Ns, delay=Bs // D, U=U, R=R, kept_energy=kept))
-    return Bank(f0=f0, M=M, slices=slices, mchirp=mchirp, T=T)
+        slices.append(Slice(rate=rate, n_taps=Hs.shape[1], delay=Bs // D, U=U, R=R, kept_energy=kept))
+    return Bank(f0=f0, M=len(mchirp), slices=slices, mchirp=mchirp, T=T)
 
 
 def build_bank(mchirp: Sequence[float], T: float, f0: int = F0_HZ, r_min: int = 32,
