@@ -623,6 +623,7 @@ struct TcPlan {
   TcReconTile *xi_dev; int *xi_begin_dev; int n_xi, xi_grid;   // xi^2 pass
   int *rbegin_dev, *cbegin_dev;
   TcCorrClass *cmaps_dev; TcCorrUnit *cunits_dev; int n_cunits, corr_grid;
+  int n_phase; std::vector<int> clist_off, clist_n;          // a2 unit lists: one per phase + one with every class
   const CorrClass *classes_dev;
   int recon_grid, recon_smem, corr_smem;
   std::vector<void *> allocs;
@@ -723,7 +724,7 @@ void tc_plan_destroy(TcPlan *p) {
 }
 
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
-                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes, int overlap, int xi_delta) {
+                   const std::vector<ReconBank> &banks, const ReconBank *, int n_det, int B, int planes, int overlap, int xi_delta, int n_phase) {
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
@@ -768,6 +769,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
       }
   }
   p->n_cunits = (int)cu.size();
+  p->n_phase = std::max(1, n_phase);
   // ---- a3: two tensor maps per bank.  Banks whose R tile fits the resident region (split mode, Kpad <= RES_KMAX) become
   //      items (bank, template tile, detector group, run of time tiles) of the resident-R kernel; the others are tiled
   //      (bank, template tile, detector, run of time tiles) for the streaming kernel
@@ -848,7 +850,21 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
   p->corr_grid = std::max(1, std::min(p->n_cunits, sms));
   std::vector<int> cbegin, rbegin;
-  lpt_assign(cu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1] + u.nt[2] + u.nt[3]) * (u.k1 - u.k0) / 128 + 128; }, cbegin);
+  {
+    // batch-ahead (a slice delayed by more than a second may be filtered ahead of need): list f holds the
+    // units of the classes correlated every push plus those whose phase is f; the last list holds every class (first push)
+    std::vector<TcCorrUnit> all;
+    for (int li = 0; li <= p->n_phase; ++li) {
+      std::vector<TcCorrUnit> lu;
+      for (const TcCorrUnit &u : cu) { const int ph = classes[u.cls].phase; if (li == p->n_phase || ph < 0 || ph == li) lu.push_back(u); }
+      std::vector<int> lb;
+      lpt_assign(lu, p->corr_grid, [](const TcCorrUnit &u) { return (long long)(u.nt[0] + u.nt[1] + u.nt[2] + u.nt[3]) * (u.k1 - u.k0) / 128 + 128; }, lb);
+      p->clist_off.push_back((int)all.size()); p->clist_n.push_back((int)lu.size());
+      all.insert(all.end(), lu.begin(), lu.end());
+      cbegin.insert(cbegin.end(), lb.begin(), lb.end());
+    }
+    cu.swap(all);
+  }
   lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, rbegin);
   std::vector<int> ibegin;
   // cost in cycles: 4 MMAs of ~97 cycles per 16 of K per tile (at least the epilogue's ~600), plus the once-per-item R load
@@ -880,12 +896,14 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   return LLOID_OK;
 }
 
-cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st) {
-  if (p->n_cunits == 0) return cudaSuccess;
+cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st, int list) {
+  if (p->clist_n[list] == 0) return cudaSuccess;
+  const TcCorrUnit *units = p->cunits_dev + p->clist_off[list];
+  const int *begin = p->cbegin_dev + (size_t)list * (p->corr_grid + 1);
   if (p->planes == 2)
-    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
+    corr_tc_kernel<2><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, units, begin, n0);
   else
-    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, p->cunits_dev, p->cbegin_dev, n0);
+    corr_tc_kernel<1><<<p->corr_grid, CORR_THREADS, p->corr_smem, st>>>(p->classes_dev, p->cmaps_dev, units, begin, n0);
   return cudaGetLastError();
 }
 

@@ -78,6 +78,8 @@ struct CorrClass {                   // slices (across banks) with identical (ra
   int nseg;
   int ylen, ncols;                   // ncols = B / D new columns per push: [n0/D + H, (n0+B)/D + H)
   float u_scale_inv;
+  int phase;                         // batch-ahead (short buffers): -1 = correlated every push; else the push index mod
+                                     // n_phase at which this class is correlated for the next n_phase pushes at once
 };
 
 struct CorrTile { int cls, row0, col0; };   // FFMA a2 work item: 64 rows x 64 columns
@@ -137,11 +139,11 @@ int tc_time_splits(int B, long long n_mtile_units);   // n_mtile_units = sum_ban
 int tc_k_segments(int Npad);  // split-K segments of the tensor-core a2 kernel for a slice of Npad taps   // partial peaks per template written by the tensor-core a3 kernel
 int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const CorrClass *classes_dev,
                    const std::vector<ReconBank> &banks, const ReconBank *banks_dev, int n_det, int B, int planes, int overlap,
-                   int xi_delta);
+                   int xi_delta, int n_phase);
 void tc_plan_destroy(TcPlan *p);
 int tc_plan_n_tt(const TcPlan *p);              // partial peaks per template and detector the a3 kernels write
 int tc_plan_recon_launches(const TcPlan *p);    // 1 or 2: streaming kernel and / or resident-R kernel
-cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st);
+cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st, int list);   // list: phase, or n_phase = every class
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank,
                             cudaStream_t st);
 cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st);

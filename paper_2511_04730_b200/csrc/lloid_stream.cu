@@ -23,6 +23,7 @@ struct lloid_stream {
   lloid_peak *peaks_hist[2];                       // xi^2: triggers of the last two pushes
   float *xi_partial_dev, *xi_den_dev;              // xi^2: [n_det][Mtot][4] numerators; [Mtot] denominators
   long long n_pushes;
+  int n_phase;                                     // batch-ahead: pushes per batch of the deep classes (1 = off)
   PeakPartial *tail_dev, *tail_partial_dev;        // overlapped trigger windows: previous buffer's tail peak, this buffer's partials
   float threshold;
   cudaStream_t st;
@@ -132,6 +133,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   const int planes = std::max(1, s->up_planes);
   s->up_chunk = std::min(B, 512);                   // = UP_CHUNK of kernels_stream.cu
   memset(s->work, 0, sizeof(s->work));
+  s->n_phase = (s->precision != LLOID_PREC_FP32_FFMA && B < s->f0 && s->f0 % B == 0 && !getenv("LLOID_DEBUG_NO_BATCH")) ? std::min(64, s->f0 / B) : 1;
   int dev = 0; cudaDeviceProp prop;
   CK(cudaGetDevice(&dev));
   CK(cudaGetDeviceProperties(&prop, dev));
@@ -204,7 +206,12 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       const RateDev &r = dp.r[rate_index[D]];
       cc.ring2 = r.ring2; cc.ring_det_stride = 2LL * r.rlen; cc.rlen = r.rlen; cc.lag = r.lag; cc.D = D;
       cc.N = (int)(emax - dmin); cc.Npad = (cc.N + 63) / 64 * 64; cc.H = kv.first.second; cc.delay = dmin;
-      cc.ncols = B / D; cc.ylen = B / D + 32; cc.u_scale_inv = 1.f;
+      cc.ncols = B / D; cc.ylen = B / D + 32; cc.u_scale_inv = 1.f; cc.phase = -1;
+      // batch-ahead: with short buffers a class whose newest tap lies more than a batch (one second) in the
+      // past is correlated once per n_phase pushes for all of them; the phases are staggered over the classes
+      if (s->n_phase > 1 && cc.delay >= (long long)(s->n_phase - 1) * (B / D) + cc.H + s->n_down + 8) {
+        cc.phase = c % s->n_phase; cc.ncols = s->n_phase * (B / D); cc.ylen = cc.ncols + B / D + 64;
+      }
       members.emplace_back();
       // keep bank order inside the class (deterministic row layout)
       std::vector<Member> mm(v.begin() + i0, v.begin() + i1);
@@ -258,10 +265,10 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     cc.yseg_stride = (long long)n_det * cc.ydet_stride;
     for (int r0 = 0; r0 < cc.Lstack; r0 += 64)
       for (int c0 = 0; c0 < cc.ncols; c0 += 64) tiles.push_back({(int)c, r0, c0});
-    s->work[0] += 2.0 * cc.Lpad * cc.Npad * cc.ncols * n_det;               // executed (padded) flop, one pass
-    s->work[2] += 2.0 * alg * cc.ncols * n_det;
+    s->work[0] += 2.0 * cc.Lpad * cc.Npad * (B / cc.D) * n_det;             // executed (padded) flop, one pass, per push
+    s->work[2] += 2.0 * alg * (B / cc.D) * n_det;
     s->work[5] += (double)cc.Lpad * cc.Npad * (s->precision == LLOID_PREC_FP32_FFMA ? 4 : 2 * planes);
-    s->work[6] += 2.0 * 4.0 * cc.Lstack * cc.ncols * n_det;
+    s->work[6] += 2.0 * 4.0 * cc.Lstack * (B / cc.D) * n_det;
   }
   CK(dev_upload(s, &s->classes_dev, s->classes));
   s->n_tiles = (int)tiles.size();
@@ -320,6 +327,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       const CorrClass &cc = s->classes[cls_of[b][i]];
       std::vector<int> key;
       key.push_back(si.D);
+      key.push_back(cc.ylen);                        // rows of batch-ahead classes live in longer Y rings: never in one item with others
       for (int h = 1; h <= si.group; ++h) key.push_back((int)std::lround(std::log2((double)bk->groups[h].f)));
       std::vector<UpRow> &dst = chains[key];
       for (int l = 0; l < si.L; ++l) {
@@ -346,8 +354,8 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
     for (size_t r0 = 0; r0 < kv.second.size(); r0 += 32) {
       UpItem it; memset(&it, 0, sizeof(it));
       it.row0 = (int)(uprows.size() + r0); it.nl = (int)std::min<size_t>(32, kv.second.size() - r0);
-      it.g = (int)key.size() - 1; it.ylen = B / key[0] + 32;
-      for (int h = 1; h <= it.g; ++h) it.log2f[h] = key[h];
+      it.g = (int)key.size() - 2; it.ylen = key[1];
+      for (int h = 1; h <= it.g; ++h) it.log2f[h] = key[h + 1];
       items.push_back(it);
     }
     uprows.insert(uprows.end(), kv.second.begin(), kv.second.end());
@@ -373,7 +381,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
   if (s->precision != LLOID_PREC_FP32_FFMA) {
-    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap, s->xi_delta);
+    int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap, s->xi_delta, s->n_phase);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
     s->n_tt = tc_plan_n_tt(s->tc);                 // partial peaks per template: the larger of the two a3 kernels' splits
     s->work[0] *= (planes == 2 ? 2 : 1);           // split mode: two MMAs per product in a2 (U_hi x, U_lo x) and in a3
@@ -425,7 +433,7 @@ extern "C" int lloid_stream_push(lloid_stream *s, const float *strain, lloid_pea
   mark(1);
   if (e == cudaSuccess) {
     where = "a2 correlate";
-    if (s->tc) e = tc_launch_corr(s->tc, s->n0_dev, s->st);
+    if (s->tc) e = tc_launch_corr(s->tc, s->n0_dev, s->st, s->n_pushes == 0 ? s->n_phase : (int)(s->n_pushes % s->n_phase));
     else e = launch_corr_ffma(s->classes_dev, s->tiles_dev, s->n_tiles, s->n_det, s->n0_dev, s->st);
   }
   mark(2);

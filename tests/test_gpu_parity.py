@@ -128,7 +128,8 @@ def test_ragged_buffer_threshold_and_host_push():
             above = ref_pk["snr"] >= thr
             assert np.array_equal(pk_host["sample"][above], ref_pk["sample"][above])
             assert np.array_equal(pk_host["snr"][above], ref_pk["snr"][above])          # same kernels: bit-identical
-            assert (pk_host["sample"][~above] == -1).all() and (pk_host["snr"][~above] == 0).all()
+            # below threshold: LLOID_NO_TRIGGER (negative samples are legitimate with trigger_overlap, include/lloid.h)
+            assert (pk_host["sample"][~above] == lib.binding.LLOID_NO_TRIGGER).all() and (pk_host["snr"][~above] == 0).all()
         st.close()
         for det in range(2):
             ref = lloid_snr(bank, strain[det])
