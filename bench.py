@@ -16,6 +16,7 @@ Prints ONE JSON line on rank 0.  `--impl reference` times the float64 CPU oracle
 """
 import argparse
 import json
+import math
 import os
 import subprocess
 import sys
@@ -443,6 +444,20 @@ def measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, K, W,
     empty_ms = float(np.median([a.elapsed_time(b) for a, b in zip(e0[8:], e1[8:])]))
     tiny.close()
 
+    # ---- event identification on the peaks of the last push (coincidence + clustering): not part of the
+    #      timed step, reported beside it
+    ev_ms = None
+    if c.n_det >= 2:
+        dt = np.full((c.n_det, c.n_det), int(math.ceil(0.0323 * f0)), dtype=np.int32)
+        np.fill_diagonal(dt, 0)
+        st.events(dt)
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        g0.record()
+        for _ in range(5):
+            lib.binding.lloid_stream_events(st.handle, st.peaks_dev.data_ptr(), dt, st.events_dev.data_ptr())
+        g1.record(); torch.cuda.synchronize()
+        ev_ms = g0.elapsed_time(g1) / 5
+
     # ---- per-stage device times (CUDA events recorded by the library on its stream) for the roofline
     st.set_stage_timing(True)
     for i in range(K):
@@ -477,6 +492,7 @@ def measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, K, W,
                        "note": "per-push device time (CUDA events around one lloid_stream_push), host time of the call, and the "
                                "device time of a push on a one-template 64-tap bank (launch overhead of the kernel sequence)"},
         "clocks": clocks, "roofline": roofline_record(cfg_no, precision, per_stage, work),
+        "events_stage_ms": ev_ms,
     }
     kept = {"cfg": cfg_no, "handles": handles, "Ms": Ms, "descr": descr, "real": keep}
     return rec, kept

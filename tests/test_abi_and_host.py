@@ -94,6 +94,21 @@ def test_null_and_state_errors_without_a_device(lib):
     assert lib.binding._lib.lloid_stream_create(C.byref(out), None, 0, 1, 2048, None) == lib.LLOID_EINVAL
     o = lib.lloid_options_default()
     assert (o.n_down, o.n_up, o.precision) == (32, 8, lib.LLOID_PREC_F16_SPLIT)
+    assert o.trigger_overlap == 0 and o.threshold == 0.0
+    # the calls around the path validate their arguments before touching a device
+    L = lib.binding._lib
+    assert L.lloid_stream_events(None, None, None, None) == lib.LLOID_EINVAL
+    assert L.lloid_stream_xi2(None, None) == lib.LLOID_EINVAL
+    assert L.lloid_bank_set_autocorrelation(None, None, 175) == lib.LLOID_EINVAL
+    assert L.lloid_xi2_series(None, 1, 1, None, None, 175, None, None) == lib.LLOID_EINVAL
+    assert L.lloid_whitener_push(None, None, None, None) == lib.LLOID_EINVAL
+    w = C.c_void_p()
+    for bad in ((1, 16384, 2000, 65536, 16384, 7, 64), (1, 16384, 2048, 65536, 16384, 6, 64), (1, 16384, 2048, 65535, 16384, 7, 64),
+                (0, 16384, 2048, 65536, 16384, 7, 64), (1, 16384, 2048, 65536, 40000, 7, 64)):
+        assert L.lloid_whitener_create(C.byref(w), *bad, None) == lib.LLOID_EINVAL and "whitener_create" in lib.lloid_last_error()
+    n = C.c_int32()
+    assert L.lloid_svd_slice(None, 4, 4, 0.9999, 4, C.byref(n), None, None, None, None, None) == lib.LLOID_EINVAL
+    assert L.lloid_whitener_hop_in(None) == -1
 
 
 def test_product_path_never_imports_the_oracle():

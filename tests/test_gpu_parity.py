@@ -304,3 +304,21 @@ def test_decimator_does_not_read_past_an_exact_size_strain_buffer(tmp_path):
     script.write_text(_TIGHT_STRAIN.format(root=root))
     r = subprocess.run([sys.executable, str(script)], capture_output=True, text=True, timeout=600)
     assert r.returncode == 0 and "TIGHT_OK" in r.stdout, (r.stdout[-1500:], r.stderr[-3000:])
+
+
+def test_streams_on_two_devices_in_one_process():
+    """Kernel attributes (dynamic shared memory opt-in) are per device: a second stream on another GPU of the same process
+    must work (process-wide `static bool attr`).  Skips on a single-GPU box."""
+    torch = _torch_cuda()
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs")
+    import paper_2511_04730_b200 as lib
+    from workloads import make_strain, random_bank
+    bank = random_bank(3, 40, [(2048, 512, 24), (1024, 768, 40), (256, 512, 33)]).as_f32()
+    x = np.stack([make_strain(5, 1024)])
+    out = []
+    for dev in ("cuda:0", "cuda:1"):
+        st = lib.LloidStream([bank], 1, 1024, device=dev)
+        out.append(st.push(x).copy())
+        st.close()
+    assert np.array_equal(out[0], out[1])
