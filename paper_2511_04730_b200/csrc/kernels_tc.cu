@@ -274,20 +274,21 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         mbar_wait(&tfull[buf], (it >> 1) & 1);
         tc_fence_after_sync();
         const uint32_t t_re = tmem + lane_base + buf * 256 + cs * 32;
+        // the slice is loaded as two halves of 16 columns: the second load is in flight while the first half is scanned
         uint32_t vr[32], vi[32];
-        tmem_ld_32x32(t_re, vr);
-        tmem_ld_32x32(t_re + 128, vi);
+        tmem_ld_32x16(t_re, *reinterpret_cast<uint32_t(*)[16]>(&vr[0]));
+        tmem_ld_32x16(t_re + 128, *reinterpret_cast<uint32_t(*)[16]>(&vi[0]));
         tmem_ld_wait();
-        tc_fence_before_sync();                        // this warp's part of the accumulators is in registers: release the buffer
-        __syncwarp();
-        if (lane == 0) mbar_arrive(&tempty[buf]);
+        tmem_ld_32x16(t_re + 16, *reinterpret_cast<uint32_t(*)[16]>(&vr[16]));
+        tmem_ld_32x16(t_re + 128 + 16, *reinterpret_cast<uint32_t(*)[16]>(&vi[16]));
         // chunk maxima are independent; the running-maximum chain is one compare + select per chunk and the record
         // stores are predicated (no vote / branch on the chain).  Only a buffer's last tile can be ragged: the masked
         // loop is a separate copy, chosen once per tile.
-        auto scan = [&](auto ragged_tag) {
+        auto scan = [&](auto ragged_tag, int c_lo, int c_hi) {
           constexpr bool RAGGED = decltype(ragged_tag)::value;
 #pragma unroll
           for (int c = 0; c < 32 / PK_CHUNK; ++c) {
+            if (c < c_lo || c >= c_hi) continue;
             const int t0c = tbase + c * PK_CHUNK;
             float p[PK_CHUNK];
 #pragma unroll
@@ -314,7 +315,14 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           }
         };
         // (t_min > 0: the tail pass of the overlapped trigger windows looks at samples [t_min, B) only)
-        if (tl.t0 + tt * TILE_N + TILE_N > B || t_min > 0) scan(std::true_type()); else scan(std::false_type());
+        const bool masked = tl.t0 + tt * TILE_N + TILE_N > B || t_min > 0;
+        constexpr int HALF_CHUNKS = 16 / PK_CHUNK;
+        if (masked) scan(std::true_type(), 0, HALF_CHUNKS); else scan(std::false_type(), 0, HALF_CHUNKS);
+        tmem_ld_wait();
+        tc_fence_before_sync();                        // this warp's part of the accumulators is in registers: release the buffer
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&tempty[buf]);
+        if (masked) scan(std::true_type(), HALF_CHUNKS, 2 * HALF_CHUNKS); else scan(std::false_type(), HALF_CHUNKS, 2 * HALF_CHUNKS);
         if (dbg) {
           float *o = snr_debug + ((size_t)det * 2 * M + 2 * m) * B;
 #pragma unroll
