@@ -133,7 +133,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   const int planes = std::max(1, s->up_planes);
   s->up_chunk = std::min(B, 512);                   // = UP_CHUNK of kernels_stream.cu
   memset(s->work, 0, sizeof(s->work));
-  s->n_phase = (s->precision != LLOID_PREC_FP32_FFMA && B < s->f0 && s->f0 % B == 0 && !getenv("LLOID_DEBUG_NO_BATCH")) ? std::min(64, s->f0 / B) : 1;
+  s->n_phase = (s->precision != LLOID_PREC_FP32_FFMA && B < s->f0 && s->f0 % B == 0) ? std::min(64, s->f0 / B) : 1;
   int dev = 0; cudaDeviceProp prop;
   CK(cudaGetDevice(&dev));
   CK(cudaGetDeviceProperties(&prop, dev));
