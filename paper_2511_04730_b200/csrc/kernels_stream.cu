@@ -134,6 +134,7 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   lane = basis row (of any slice / bank with that chain: UpRow gives its source ring row and destination column).
 // ------------------------------------------------------------------------------------------------
 #define UP_RUN 8
+#define UP_LD 8      // ring columns loaded per round and warp
 #define UP_CHUNK 512  // f0 samples per CTA
 #define UP_MAXW (UP_CHUNK / 2 + 40)   // widest staged level: chunk/2 + 2*8 + 1 (+ slack)
 template <int HALF_PLANES>
@@ -189,22 +190,23 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
   const float *yr = rw->ysrc + (size_t)det * rw->ydet_stride;
   const int nseg = rw->nseg;
   const size_t yseg = (size_t)rw->yseg_stride;
-  // 4 ring columns at a time: all (column, tap segment) loads are issued before any add; the split-K partial sums are
-  // then added in segment order (deterministic, same order for every caller)
-  auto load_y4 = [&](const int (&sl)[4], const bool (&ok)[4], float (&v)[4]) {
+  // UP_LD ring columns at a time: all (column, tap segment) loads are issued before any add (the kernel is latency-bound:
+  // memory-level parallelism is what the load phase needs); the split-K partial sums are then added in segment order
+  // (deterministic, same order for every caller)
+  auto load_yn = [&](const int (&sl)[UP_LD], const bool (&ok)[UP_LD], float (&v)[UP_LD]) {
 #pragma unroll
-    for (int i = 0; i < 4; ++i) v[i] = 0.f;
-    for (int sg0 = 0; sg0 < nseg; sg0 += 4) {
-      float t[4][4];
+    for (int i = 0; i < UP_LD; ++i) v[i] = 0.f;
+    for (int sg0 = 0; sg0 < nseg; sg0 += 2) {
+      float t[UP_LD][2];
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
+      for (int j = 0; j < 2; ++j)
 #pragma unroll
-        for (int i = 0; i < 4; ++i)
-          t[i][j] = (ok[i] && sg0 + j < nseg) ? yr[(size_t)(sg0 + j) * yseg + (size_t)sl[i] * ypitch] : 0.f;
+        for (int i = 0; i < UP_LD; ++i)
+          t[i][j] = (ok[i] && sg0 + j < nseg) ? __ldg(yr + (size_t)(sg0 + j) * yseg + (size_t)sl[i] * ypitch) : 0.f;
 #pragma unroll
-      for (int j = 0; j < 4; ++j)
+      for (int j = 0; j < 2; ++j)
 #pragma unroll
-        for (int i = 0; i < 4; ++i) v[i] += t[i][j];
+        for (int i = 0; i < UP_LD; ++i) v[i] += t[i][j];
     }
   };
   void *yup = rw->yup;
@@ -215,36 +217,26 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
   const int wg = s_w[G];
   int slot = s_slot0 + warp;
   if (slot >= ylen) slot -= ylen;
-  if (G == 0) {
-    for (int c = warp; c < wg; c += 4 * nwarp) {
-      float v[4];
-      int sl[4];
-      bool ok[4];
+  for (int c = warp; c < wg; c += UP_LD * nwarp) {
+    float v[UP_LD];
+    int sl[UP_LD];
+    bool ok[UP_LD];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        sl[i] = slot; ok[i] = active && c + i * nwarp < wg;
-        slot += nwarp; if (slot >= ylen) slot -= ylen;
-      }
-      load_y4(sl, ok, v);
-#pragma unroll
-      for (int i = 0; i < 4; ++i)
-        if (active && c + i * nwarp < wg) up_store<HALF_PLANES>(yup, out0 + (size_t)(c + i * nwarp) * kpitch, plane_stride, v[i]);
-    }
-    return;
-  }
-  for (int c = warp; c < wg; c += 4 * nwarp) {            // 4 independent loads in flight per warp
-    float v[4];
-    int sl[4];
-    bool ok[4];
-#pragma unroll
-    for (int i = 0; i < 4; ++i) {
+    for (int i = 0; i < UP_LD; ++i) {
       sl[i] = slot; ok[i] = active && c + i * nwarp < wg;
       slot += nwarp; if (slot >= ylen) slot -= ylen;
     }
-    load_y4(sl, ok, v);
+    load_yn(sl, ok, v);
+    if (G == 0) {                                          // full-rate rows: converted and stored as they are
 #pragma unroll
-    for (int i = 0; i < 4; ++i) if (c + i * nwarp < wg) buf[0][c + i * nwarp][lane] = v[i];
+      for (int i = 0; i < UP_LD; ++i)
+        if (ok[i]) up_store<HALF_PLANES>(yup, out0 + (size_t)(c + i * nwarp) * kpitch, plane_stride, v[i]);
+    } else {
+#pragma unroll
+      for (int i = 0; i < UP_LD; ++i) if (c + i * nwarp < wg) buf[0][c + i * nwarp][lane] = v[i];
+    }
   }
+  if (G == 0) return;
   __syncthreads();
   int cur = 0;
   for (int h = G; h >= 1; --h) {
