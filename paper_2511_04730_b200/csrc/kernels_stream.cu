@@ -131,42 +131,94 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   Stage h -> h-1 with factor f:  out[i] = in[i/f] if i mod f == 0 (Eq. 8 case 1), else
 //   sum_{k=0}^{15} in[floor(i/f) + 8 - k] * g_f[k f + (i mod f)]   (Eq. 7-8, zero-phase form).
 //   CTA = (time chunk of `chunk` f0 samples, item = 32 basis rows sharing one upsample chain, detector).
-//   lane = basis row (of any slice / bank with that chain: UpRow gives its source ring row and destination column).
+//   lane = basis row (of any slice / bank with that chain: UpRow gives its source ring row and destination row).
+//   Output, tensor-core modes (HALF_PLANES 1 / 2): one row of samples per basis row (fp16 plane; correction plane = two byte
+//   rows per basis row).  A store instruction that fills only part of a 32-byte sector costs as much as 2-3 full ones
+//   (measured: 1.3-3.0 TB/s against 6.3-7.4), and rows of one chain are never 16 neighbours on the basis axis -- so the
+//   samples of a row are contiguous and the CTA stages UP_TT samples x 32 rows in shared memory, then writes them with
+//   16-byte vectors, whole sectors only.  FFMA mode (HALF_PLANES 0) keeps fp32 [sample][Kpad] and stores directly.
 // ------------------------------------------------------------------------------------------------
 #define UP_RUN 8
 #define UP_LD 8      // ring columns loaded per round and warp
 #define UP_CHUNK 512  // f0 samples per CTA
 #define UP_MAXW (UP_CHUNK / 2 + 40)   // widest staged level: chunk/2 + 2*8 + 1 (+ slack)
+#define UP_TT 256                     // samples per output tile (tensor-core layouts)
+#define UP_P16 (UP_TT * 2 + 16)       // tile row pitches in bytes: odd multiples of 16, so 16-byte accesses by lane = row do not conflict
+#define UP_P8 (UP_TT + 16)
+#define UP_T8 (32 * UP_P16)           // byte rows start here: row = term * 32 + lane
+static_assert(UP_T8 + 64 * UP_P8 <= UP_MAXW * 32 * 4, "the output tile must fit one staging buffer");
+
+// the two correction bytes of DESIGN.md section 4 for a value v whose fp16 rounding is hf: e5m2(4 (v - hf)), e5m2(hf / 256)
+__device__ __forceinline__ unsigned short up_pair_lo(float v0, float h0, float v1, float h1) {
+  return __nv_cvt_float2_to_fp8x2(make_float2((v0 - h0) * 4.f, (v1 - h1) * 4.f), __NV_SATFINITE, __NV_E5M2);
+}
+__device__ __forceinline__ unsigned short up_pair_hi(float h0, float h1) {
+  return __nv_cvt_float2_to_fp8x2(make_float2(h0 * (1.f / 256.f), h1 * (1.f / 256.f)), __NV_SATFINITE, __NV_E5M2);
+}
+// one sample of row `lane` into the tile
 template <int HALF_PLANES>
-__device__ __forceinline__ void up_store(void *yup, size_t o, size_t plane_stride, float v) {
-  if (HALF_PLANES == 0) {
-    reinterpret_cast<float *>(yup)[o] = v;
-  } else {
-    __half hi16 = __float2half_rn(v);
-    reinterpret_cast<__half *>(yup)[o] = hi16;
-    if (HALF_PLANES == 2) {
-      // correction plane: 16 bits = { e5m2(4 Y_lo), e5m2(Y_hi / 256) }, B operand of the fp8 MMA of a3
-      const float hf = __half2float(hi16);
-      reinterpret_cast<unsigned short *>(yup)[o + plane_stride] =
-          __nv_cvt_float2_to_fp8x2(make_float2((v - hf) * 4.f, hf * (1.f / 256.f)), __NV_SATFINITE, __NV_E5M2);
-    }
+__device__ __forceinline__ void tile_put(unsigned char *tile, int lane, int tc, float v) {
+  const __half h = __float2half_rn(v);
+  *reinterpret_cast<__half *>(tile + lane * UP_P16 + tc * 2) = h;
+  if (HALF_PLANES == 2) {
+    const float hf = __half2float(h);
+    tile[UP_T8 + lane * UP_P8 + tc] = (unsigned char)__nv_cvt_float_to_fp8((v - hf) * 4.f, __NV_SATFINITE, __NV_E5M2);
+    tile[UP_T8 + (32 + lane) * UP_P8 + tc] = (unsigned char)__nv_cvt_float_to_fp8(hf * (1.f / 256.f), __NV_SATFINITE, __NV_E5M2);
   }
 }
+// eight consecutive samples (tc a multiple of 8): one 16-byte and two 8-byte shared stores
+template <int HALF_PLANES>
+__device__ __forceinline__ void tile_put8(unsigned char *tile, int lane, int tc, const float (&v)[8]) {
+  uint32_t w[4], a[2], b[2];
+  unsigned short pa[4], pb[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const __half2 h2 = __floats2half2_rn(v[2 * i], v[2 * i + 1]);
+    w[i] = *reinterpret_cast<const uint32_t *>(&h2);
+    if (HALF_PLANES == 2) {
+      const float2 f = __half22float2(h2);
+      pa[i] = up_pair_lo(v[2 * i], f.x, v[2 * i + 1], f.y);
+      pb[i] = up_pair_hi(f.x, f.y);
+    }
+  }
+  *reinterpret_cast<uint4 *>(tile + lane * UP_P16 + tc * 2) = make_uint4(w[0], w[1], w[2], w[3]);
+  if (HALF_PLANES == 2) {
+    a[0] = pa[0] | ((uint32_t)pa[1] << 16); a[1] = pa[2] | ((uint32_t)pa[3] << 16);
+    b[0] = pb[0] | ((uint32_t)pb[1] << 16); b[1] = pb[2] | ((uint32_t)pb[3] << 16);
+    *reinterpret_cast<uint2 *>(tile + UP_T8 + lane * UP_P8 + tc) = make_uint2(a[0], a[1]);
+    *reinterpret_cast<uint2 *>(tile + UP_T8 + (32 + lane) * UP_P8 + tc) = make_uint2(b[0], b[1]);
+  }
+}
+// FFMA mode: fp32 [sample][Kpad]
+__device__ __forceinline__ void up_store_f32(void *yup, size_t o, float v) { reinterpret_cast<float *>(yup)[o] = v; }
 
 template <int HALF_PLANES>
 __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
                                                           const float *__restrict__ uptaps,
                                                           const int *__restrict__ uptap_off,
                                                           const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
+  static_assert(UP_LD == 8, "tile_put8 takes the UP_LD columns of one load round");
   extern __shared__ __align__(16) float up_dyn[];
   float(*buf)[UP_MAXW][32] = reinterpret_cast<float(*)[UP_MAXW][32]>(up_dyn);
   __shared__ int s_r0[LLOID_MAX_GROUPS + 1], s_w[LLOID_MAX_GROUPS + 1], s_lf[LLOID_MAX_GROUPS + 1], s_slot0;
+  __shared__ unsigned char *s_dst16[32], *s_dst8[32];     // tensor-core layouts: where sample ka of each lane's row goes
   const UpItem *it = &items[blockIdx.y];
   const int det = blockIdx.z;
   const int ka = blockIdx.x * chunk;
   const int kb = min(ka + chunk, B);
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
-  const int G = it->g;
+  const int G = it->g, nl = it->nl;
+  const bool active = lane < nl;
+  const UpRow *rw = &rows[it->row0 + (active ? lane : 0)];     // this lane's row: source ring row and destination
+  const int ylen = it->ylen, ypitch = rw->ypitch;
+  const int kpitch = rw->kpitch;                               // FFMA: Kpad (sample pitch); tensor-core layouts: yup_pitch(B) (row pitch)
+  void *yup = rw->yup;
+  const size_t rowoff = (size_t)det * rw->yup_det_stride + (size_t)rw->dst0;
+  const size_t out0 = rowoff + (size_t)ka * kpitch;            // FFMA: element (sample ka, this row's column)
+  if (HALF_PLANES > 0 && warp == 0) {
+    s_dst16[lane] = reinterpret_cast<unsigned char *>(yup) + 2 * (rowoff + ka);
+    s_dst8[lane] = reinterpret_cast<unsigned char *>(yup) + 2 * ((size_t)rw->yup_plane_stride + rowoff) + ka;
+  }
   // Level h covers the absolute index range [lo_h, hi_h) at its rate (64-bit, thread 0 only); everything the
   // loops below need is relative and fits 32 bits: width w_h, phase r0_h = lo_{h-1} mod f_h of the first output of
   // stage h, and the Y-ring slot of column lo_G.  lo_h = floor(lo_{h-1} / f_h) - 8, hi_h = floor((hi_{h-1} - 1) / f_h) + 9.
@@ -181,21 +233,25 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
       hi = ((hi - 1) >> lf) + LLOID_NUP + 1;
       s_w[h] = (int)(hi - lo);
     }
-    s_slot0 = (int)((lo + 64) % it->ylen);
+    s_slot0 = (int)((lo + 64) % ylen);
   }
   __syncthreads();
-  const bool active = lane < it->nl;
-  const UpRow *rw = &rows[it->row0 + (active ? lane : 0)];     // this lane's row: source ring row and destination column
-  const int ylen = it->ylen, ypitch = rw->ypitch, kpitch = rw->kpitch;
   const float *yr = rw->ysrc + (size_t)det * rw->ydet_stride;
   const int nseg = rw->nseg;
   const size_t yseg = (size_t)rw->yseg_stride;
-  // UP_LD ring columns at a time: all (column, tap segment) loads are issued before any add (the kernel is latency-bound:
-  // memory-level parallelism is what the load phase needs); the split-K partial sums are then added in segment order
-  // (deterministic, same order for every caller)
-  auto load_yn = [&](const int (&sl)[UP_LD], const bool (&ok)[UP_LD], float (&v)[UP_LD]) {
+  // UP_LD consecutive ring columns from c0 on: all (column, tap segment) loads are issued before any add (memory-level
+  // parallelism is what the load phase needs); the split-K partial sums are then added in segment order (deterministic,
+  // the same order for every caller).  Columns never computed at stream start are the ring's zeros.
+  auto load_yn = [&](int c0, int c_end, float (&v)[UP_LD]) {
+    int sl[UP_LD];
+    bool ok[UP_LD];
+    const int slot = (s_slot0 + c0) % ylen;
 #pragma unroll
-    for (int i = 0; i < UP_LD; ++i) v[i] = 0.f;
+    for (int i = 0; i < UP_LD; ++i) {
+      sl[i] = slot + i >= ylen ? slot + i - ylen : slot + i;
+      ok[i] = active && c0 + i < c_end;
+      v[i] = 0.f;
+    }
     for (int sg0 = 0; sg0 < nseg; sg0 += 2) {
       float t[UP_LD][2];
 #pragma unroll
@@ -209,90 +265,108 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
         for (int i = 0; i < UP_LD; ++i) v[i] += t[i][j];
     }
   };
-  void *yup = rw->yup;
-  const size_t plane_stride = (size_t)rw->yup_plane_stride;
-  const size_t out0 = (size_t)det * rw->yup_det_stride + (size_t)rw->dst0 + (size_t)ka * kpitch;   // sample ka
+  // tile -> global: 16-byte vectors, a warp instruction covers 256 samples of one fp16 row / 2 x 256 of two byte rows
+  auto flush = [&](const unsigned char *tile, int c_lo, int ncol) {
+    for (int r = warp; r < nl; r += nwarp) {
+      const int tc = lane * 8;
+      unsigned char *dst = s_dst16[r] + 2 * (c_lo + tc);
+      const unsigned char *src = tile + r * UP_P16 + 2 * tc;
+      if (tc + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+      else
+        for (int j = 0; j < 8; ++j)
+          if (tc + j < ncol) reinterpret_cast<unsigned short *>(dst)[j] = reinterpret_cast<const unsigned short *>(src)[j];
+    }
+    if (HALF_PLANES == 2) {
+      for (int rr = 2 * warp + (lane >> 4); rr < 64; rr += 2 * nwarp) {      // rr = term * 32 + row
+        const int r = rr & 31, tc = (lane & 15) * 16;
+        if (r < nl) {
+          unsigned char *dst = s_dst8[r] + (size_t)(rr >> 5) * kpitch + c_lo + tc;
+          const unsigned char *src = tile + UP_T8 + rr * UP_P8 + tc;
+          if (tc + 16 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+          else
+            for (int j = 0; j < 16; ++j)
+              if (tc + j < ncol) dst[j] = src[j];
+        }
+      }
+    }
+  };
 
-  // level G from the Y ring (columns never computed at stream start are the ring's zeros)
-  const int wg = s_w[G];
-  int slot = s_slot0 + warp;
-  if (slot >= ylen) slot -= ylen;
-  for (int c = warp; c < wg; c += UP_LD * nwarp) {
-    float v[UP_LD];
-    int sl[UP_LD];
-    bool ok[UP_LD];
+  if (G == 0) {                                              // full-rate rows: converted and stored as they are
+    const int w0 = s_w[0];
+    if (HALF_PLANES == 0) {
+      for (int c0 = warp * UP_LD; c0 < w0; c0 += UP_LD * nwarp) {
+        float v[UP_LD];
+        load_yn(c0, w0, v);
 #pragma unroll
-    for (int i = 0; i < UP_LD; ++i) {
-      sl[i] = slot; ok[i] = active && c + i * nwarp < wg;
-      slot += nwarp; if (slot >= ylen) slot -= ylen;
-    }
-    load_yn(sl, ok, v);
-    if (G == 0) {                                          // full-rate rows: converted and stored as they are
-#pragma unroll
-      for (int i = 0; i < UP_LD; ++i)
-        if (ok[i]) up_store<HALF_PLANES>(yup, out0 + (size_t)(c + i * nwarp) * kpitch, plane_stride, v[i]);
+        for (int i = 0; i < UP_LD; ++i)
+          if (active && c0 + i < w0) up_store_f32(yup, out0 + (size_t)(c0 + i) * kpitch, v[i]);
+      }
     } else {
+      unsigned char *tile = reinterpret_cast<unsigned char *>(buf[0]);
+      for (int c_lo = 0; c_lo < w0; c_lo += UP_TT) {
+        const int c_hi = min(c_lo + UP_TT, w0);
+        for (int c0 = c_lo + warp * UP_LD; c0 < c_hi; c0 += UP_LD * nwarp) {
+          float v[UP_LD];
+          load_yn(c0, c_hi, v);
+          if (c0 + UP_LD <= c_hi) tile_put8<HALF_PLANES>(tile, lane, c0 - c_lo, v);
+          else {
 #pragma unroll
-      for (int i = 0; i < UP_LD; ++i) if (c + i * nwarp < wg) buf[0][c + i * nwarp][lane] = v[i];
+            for (int i = 0; i < UP_LD; ++i)
+              if (c0 + i < c_hi) tile_put<HALF_PLANES>(tile, lane, c0 + i - c_lo, v[i]);
+          }
+        }
+        __syncthreads();
+        flush(tile, c_lo, c_hi - c_lo);
+        if (c_hi < w0) __syncthreads();
+      }
     }
+    return;
   }
-  if (G == 0) return;
+
+  // level G from the Y ring
+  const int wg = s_w[G];
+  for (int c0 = warp * UP_LD; c0 < wg; c0 += UP_LD * nwarp) {
+    float v[UP_LD];
+    load_yn(c0, wg, v);
+#pragma unroll
+    for (int i = 0; i < UP_LD; ++i)
+      if (c0 + i < wg) buf[0][c0 + i][lane] = v[i];
+  }
   __syncthreads();
+  // The run of one warp: UP_RUN consecutive inputs qq = q0 + u of a stage, held in registers with their 15 neighbours:
+  // in[qq + 8 - k] = X[u + 15 - k] (in[qq] sits at buffer index qq + 8): ~3 shared loads per 16 FMA, no per-tap index arithmetic.
+  // x2 stage: taps g_2[2k+1] come from the kernel parameter (constant bank), FFMA with a constant operand.
+#define UP_LOAD_RUN()                                                                              \
+  const int nrun = min(UP_RUN, qb - q0);                                                           \
+  float X[UP_RUN + 15];                                                                            \
+  _Pragma("unroll") for (int j = 0; j < UP_RUN + 15; ++j) X[j] = (j < nrun + 15) ? in[q0 + 1 + j][lane] : 0.f; \
+  const int cbase = (q0 << lf) - r0;                        /* output index of (u = 0, phase 0) */
+#define UP_ODD_X2()                                                                                \
+  float odd[UP_RUN];                                                                               \
+  _Pragma("unroll") for (int u = 0; u < UP_RUN; ++u) {                                             \
+    float v0 = 0.f, v1 = 0.f;                                                                      \
+    _Pragma("unroll") for (int k = 0; k < 16; k += 2) {                                            \
+      v0 = fmaf(X[u + 15 - k], taps2.t[k], v0);                                                    \
+      v1 = fmaf(X[u + 14 - k], taps2.t[k + 1], v1);                                                \
+    }                                                                                              \
+    odd[u] = v0 + v1;                                                                              \
+  }
+
   int cur = 0;
-  for (int h = G; h >= 1; --h) {
+  for (int h = G; h >= 2; --h) {                             // stages that stay in shared memory
     const int lf = s_lf[h], f = 1 << lf, r0 = s_r0[h], wout = s_w[h - 1];
     // Output c (relative to lo_{h-1}) has input index qq = (r0 + c) >> lf relative to floor(lo_{h-1}/f) and phase
-    // (r0 + c) & (f-1); in[qq] sits at buffer index qq + 8.  Each warp takes a run of consecutive qq, UP_RUN at a time,
-    // with the run's inputs held in registers: ~3 shared loads per 16 FMA, no per-tap index arithmetic.
-    // runs of UP_RUN inputs per warp (a multiple of UP_RUN each, so only the last warp's last run is ragged)
+    // (r0 + c) & (f-1).  Each warp takes consecutive qq in runs of UP_RUN (a multiple of UP_RUN per warp, so only the
+    // last warp's last run is ragged).
     const int nq = ((r0 + wout - 1) >> lf) + 1, per = ((nq + nwarp - 1) / nwarp + UP_RUN - 1) / UP_RUN * UP_RUN;
     const int qa = warp * per, qb = min(qa + per, nq);
     const float(*in)[32] = buf[cur];
     float(*out)[32] = buf[cur ^ 1];
     for (int q0 = qa; q0 < qb; q0 += UP_RUN) {
-      // the run's inputs in[q0 - 7 .. q0 + UP_RUN + 7] (buffer index q0 + 1 + j) held in registers:
-      // in[qq + 8 - k] = X[u + 15 - k] for qq = q0 + u
-      const int nrun = min(UP_RUN, qb - q0);
-      float X[UP_RUN + 15];
-#pragma unroll
-      for (int j = 0; j < UP_RUN + 15; ++j) X[j] = (j < nrun + 15) ? in[q0 + 1 + j][lane] : 0.f;
-      const int cbase = (q0 << lf) - r0;                    // output index of (u = 0, phase 0)
+      UP_LOAD_RUN()
       if (f == 2) {
-        // taps g_2[2k+1] come from the kernel parameter (constant bank): FFMA with a constant operand
-        float odd[UP_RUN];
-#pragma unroll
-        for (int u = 0; u < UP_RUN; ++u) {
-          float v0 = 0.f, v1 = 0.f;
-#pragma unroll
-          for (int k = 0; k < 16; k += 2) {
-            v0 = fmaf(X[u + 15 - k], taps2.t[k], v0);
-            v1 = fmaf(X[u + 14 - k], taps2.t[k + 1], v1);
-          }
-          odd[u] = v0 + v1;
-        }
-        const bool full = nrun == UP_RUN && cbase >= 0 && cbase + 2 * UP_RUN <= wout;    // warp-uniform
-        if (h == 1) {
-          size_t o = out0 + (size_t)max(cbase, 0) * kpitch;
-          if (full) {
-            if (active) {
-#pragma unroll
-              for (int u = 0; u < UP_RUN; ++u) {
-                up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]);
-                up_store<HALF_PLANES>(yup, o + kpitch, plane_stride, odd[u]);
-                o += 2 * (size_t)kpitch;
-              }
-            }
-          } else {
-#pragma unroll
-            for (int u = 0; u < UP_RUN; ++u) {
-              const int c0 = cbase + 2 * u;
-              if (u < nrun && active) {
-                if (c0 >= 0 && c0 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, X[u + 7]); o += kpitch; }
-                if (c0 + 1 >= 0 && c0 + 1 < wout) { up_store<HALF_PLANES>(yup, o, plane_stride, odd[u]); o += kpitch; }
-              }
-            }
-          }
-        } else if (full) {
+        UP_ODD_X2()
+        if (nrun == UP_RUN && cbase >= 0 && cbase + 2 * UP_RUN <= wout) {    // warp-uniform
 #pragma unroll
           for (int u = 0; u < UP_RUN; ++u) {
             out[cbase + 2 * u][lane] = X[u + 7];                                 // phase 0: the copy of Eq. 8 case 1
@@ -324,10 +398,7 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
                 }
               }
               const int c = cbase + (u << lf) + ph;
-              if (c >= 0 && c < wout) {
-                if (h == 1) { if (active) up_store<HALF_PLANES>(yup, out0 + (size_t)c * kpitch, plane_stride, v0 + v1); }
-                else out[c][lane] = v0 + v1;
-              }
+              if (c >= 0 && c < wout) out[c][lane] = v0 + v1;
             }
           }
         }
@@ -336,6 +407,87 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
     __syncthreads();
     cur ^= 1;
   }
+
+  // last stage (to f0).  FFMA mode stores every output directly; the tensor-core layouts go through the tile, UP_TT output
+  // samples at a time (the staging buffer not read by this stage), every warp taking its share of each tile's runs.
+  {
+    const int lf = s_lf[1], f = 1 << lf, r0 = s_r0[1], wout = s_w[0];
+    const float(*in)[32] = buf[cur];
+    unsigned char *tile = reinterpret_cast<unsigned char *>(buf[cur ^ 1]);
+    const float *g = uptaps + uptap_off[lf];
+    const int tt = HALF_PLANES == 0 ? wout : UP_TT;
+    for (int c_lo = 0; c_lo < wout; c_lo += tt) {
+      const int c_hi = min(c_lo + tt, wout);
+      const int q_lo = (r0 + c_lo) >> lf, q_hi = ((r0 + c_hi - 1) >> lf) + 1;
+      const int per = ((q_hi - q_lo + nwarp - 1) / nwarp + UP_RUN - 1) / UP_RUN * UP_RUN;
+      const int qa = q_lo + warp * per, qb = min(qa + per, q_hi);
+      for (int q0 = qa; q0 < qb; q0 += UP_RUN) {
+        UP_LOAD_RUN()
+        if (f == 2) {
+          UP_ODD_X2()
+          const bool full = nrun == UP_RUN && cbase >= c_lo && cbase + 2 * UP_RUN <= c_hi;    // warp-uniform
+          if (HALF_PLANES == 0) {
+            if (active) {
+#pragma unroll
+              for (int u = 0; u < UP_RUN; ++u) {
+                const int c0 = cbase + 2 * u;
+                if (u < nrun) {
+                  if (full || (c0 >= c_lo && c0 < c_hi)) up_store_f32(yup, out0 + (size_t)c0 * kpitch, X[u + 7]);
+                  if (full || (c0 + 1 >= c_lo && c0 + 1 < c_hi)) up_store_f32(yup, out0 + (size_t)(c0 + 1) * kpitch, odd[u]);
+                }
+              }
+            }
+          } else if (full && ((cbase - c_lo) & 7) == 0) {
+#pragma unroll
+            for (int hh = 0; hh < 2; ++hh) {
+              float v[8];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { v[2 * u] = X[4 * hh + u + 7]; v[2 * u + 1] = odd[4 * hh + u]; }
+              tile_put8<HALF_PLANES>(tile, lane, cbase - c_lo + 8 * hh, v);
+            }
+          } else {
+#pragma unroll
+            for (int u = 0; u < UP_RUN; ++u) {
+              const int c0 = cbase + 2 * u;
+              if (u < nrun) {
+                if (c0 >= c_lo && c0 < c_hi) tile_put<HALF_PLANES>(tile, lane, c0 - c_lo, X[u + 7]);
+                if (c0 + 1 >= c_lo && c0 + 1 < c_hi) tile_put<HALF_PLANES>(tile, lane, c0 + 1 - c_lo, odd[u]);
+              }
+            }
+          }
+        } else {
+#pragma unroll
+          for (int u = 0; u < UP_RUN; ++u) {
+            if (u < nrun) {
+              for (int ph = 0; ph < f; ++ph) {
+                float v0 = 0.f, v1 = 0.f;
+                if (ph == 0) v0 = X[u + 7];
+                else {
+#pragma unroll
+                  for (int k = 0; k < 16; k += 2) {
+                    v0 = fmaf(X[u + 15 - k], g[k * f + ph], v0);
+                    v1 = fmaf(X[u + 14 - k], g[(k + 1) * f + ph], v1);
+                  }
+                }
+                const int c = cbase + (u << lf) + ph;
+                if (c >= c_lo && c < c_hi) {
+                  if (HALF_PLANES == 0) { if (active) up_store_f32(yup, out0 + (size_t)c * kpitch, v0 + v1); }
+                  else tile_put<HALF_PLANES>(tile, lane, c - c_lo, v0 + v1);
+                }
+              }
+            }
+          }
+        }
+      }
+      if (HALF_PLANES > 0) {
+        __syncthreads();
+        flush(tile, c_lo, c_hi - c_lo);
+        if (c_hi < wout) __syncthreads();
+      }
+    }
+  }
+#undef UP_LOAD_RUN
+#undef UP_ODD_X2
 }
 
 // Per-device kernel attributes (dynamic shared memory opt-in) and the x2 taps: called by every lloid_stream_create on
@@ -421,8 +573,12 @@ __global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_d
 // xi^2 support: copy this push's upsampled Y into slot `slot` of the three-buffer history ring (16-byte vectors)
 __global__ void yup_copy_kernel(const YupCopy *__restrict__ table, int slot) {
   const YupCopy c = table[blockIdx.y];
-  uint4 *dst = c.dst + (long long)slot * c.dst_slot_stride16;
-  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < c.n16; i += (long long)gridDim.x * blockDim.x) dst[i] = c.src[i];
+  uint4 *dst = c.dst + (long long)slot * c.row16;            // rows of 3 B samples: this push's B samples go to columns slot * B ...
+  const long long n16 = c.n_rows * c.row16;
+  for (long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x; i < n16; i += (long long)gridDim.x * blockDim.x) {
+    const long long r = i / c.row16;
+    dst[r * c.dst_pitch16 + (i - r * c.row16)] = c.src[i];
+  }
 }
 cudaError_t launch_yup_copy(const YupCopy *table_dev, int n_pieces, int slot, cudaStream_t st) {
   if (n_pieces == 0) return cudaSuccess;

@@ -40,9 +40,11 @@ static constexpr int RECON_SMEM_BUDGET = 232448 - 1024 - 256;   // dynamic share
 struct TcReconTile { int bank, det, ndet, m0, t0, nt, slot; };   // detectors det..det+ndet-1 x nt consecutive time tiles from sample t0; partial slot
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
   CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle (resident variant)
-  CUtensorMap mapY;                          // [planes*n_det*B rows][Kpad] fp16, box 32 x 128, 64-byte swizzle
-  CUtensorMap mapR64, mapY64;                // the same arrays, box 64 x 128, 128-byte swizzle (streaming variant)
-  CUtensorMap mapYh;                         // xi^2: [planes*n_det*3B rows][Kpad] history ring of upsampled Y, box 64 x 128
+  CUtensorMap mapR64;                        // the same array, box 64 x 128, 128-byte swizzle (streaming variant)
+  // upsampled Y, sample-contiguous rows: plane 0 fp16 [n_det*Kpad rows][Bp], boxes of 64 samples x
+  // 32 / 64 rows; correction plane bytes [n_det*2*Kpad rows][Bp], boxes of 128 samples x 64 / 128 rows; 128-byte swizzle
+  CUtensorMap mapY, mapY64, mapY8, mapY8_64;
+  CUtensorMap mapYh, mapYh8;                 // xi^2: the history ring, rows of 3 B samples, boxes of the streaming variant
   const float2 *acorr;                       // xi^2: [M][2 xi_delta + 1] autocorrelations
   int M, Mpad, Kpad, tmpl_off;
   float inv_scale;
@@ -120,29 +122,32 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         }
         for (int d = 0; d < tl.ndet; ++d)
         for (int tt = 0; tt < tl.nt; ++tt) {
-          int yrow = (tl.det + d) * B + tl.t0 + tt * TILE_N;
-          int yplane = n_det * B;                                  // rows between the planes of the Y array
+          int ycol = tl.t0 + tt * TILE_N;                          // first sample of the tile = innermost TMA coordinate
+          const int yrow = (tl.det + d) * bk->Kpad;                // first row of the detector in the fp16 plane (x2 in the byte plane)
           if (XI) {
-            // history ring: sample t of the target buffer sits at row (row_base + t) mod ring_rows (t may be negative)
-            int r = (xi.row_base + tl.t0 + tt * TILE_N) % xi.ring_rows;
-            if (r < 0) r += xi.ring_rows;
-            yrow = (tl.det + d) * xi.ring_rows + r;
-            yplane = n_det * xi.ring_rows;
+            // history ring: sample t of the target buffer sits at column (row_base + t) mod ring_rows (t may be negative)
+            ycol = (xi.row_base + ycol) % xi.ring_rows;
+            if (ycol < 0) ycol += xi.ring_rows;
           }
           for (int kb = 0; kb < nkb; ++kb) {
             mbar_wait(&empty[stage], phase ^ 1);
             mbar_arrive_expect_tx(&full[stage], STAGE_BYTES);
             uint8_t *sdst = ring + stage * STAGE_BYTES;
+            // Y tile = two boxes of 64 samples x RBK rows (fp16) / one box of 128 samples x 2 RBK rows (correction bytes)
             if (RES) {
-              tma_load_2d(sdst, &bk->mapY, &full[stage], kb * RBK, yrow);
-              tma_load_2d(sdst + RTILE_BYTES, &bk->mapY, &full[stage], kb * RBK, n_det * B + yrow);
+              tma_load_2d(sdst, &bk->mapY, &full[stage], ycol, yrow + kb * RBK);
+              tma_load_2d(sdst + RTILE_BYTES / 2, &bk->mapY, &full[stage], ycol + 64, yrow + kb * RBK);
+              tma_load_2d(sdst + RTILE_BYTES, &bk->mapY8, &full[stage], ycol, 2 * (yrow + kb * RBK));
             } else {
 #pragma unroll
               for (int p = 0; p < PLANES; ++p) {
                 tma_load_2d(sdst + (3 * p + 0) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 0) * bk->Mpad + tl.m0);
                 tma_load_2d(sdst + (3 * p + 1) * RTILE_BYTES, &bk->mapR64, &full[stage], kb * RBK, (p * 2 + 1) * bk->Mpad + tl.m0);
-                tma_load_2d(sdst + (3 * p + 2) * RTILE_BYTES, XI ? &bk->mapYh : &bk->mapY64, &full[stage], kb * RBK, p * yplane + yrow);
               }
+              const CUtensorMap *my = XI ? &bk->mapYh : &bk->mapY64, *my8 = XI ? &bk->mapYh8 : &bk->mapY8_64;
+              tma_load_2d(sdst + 2 * RTILE_BYTES, my, &full[stage], ycol, yrow + kb * RBK);
+              tma_load_2d(sdst + 2 * RTILE_BYTES + RTILE_BYTES / 2, my, &full[stage], ycol + 64, yrow + kb * RBK);
+              if (PLANES == 2) tma_load_2d(sdst + 5 * RTILE_BYTES, my8, &full[stage], ycol, 2 * (yrow + kb * RBK));
             }
             if (++stage == STAGES) { stage = 0; phase ^= 1; }
           }
@@ -152,10 +157,13 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
   } else if (warp == 1) {
     // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers),
     // one elected lane issues the MMAs of a K block and the commits
-    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N), idesc8 = idesc_f8_f32(TILE_M, TILE_N);
+    // R (A operand) is K-major, upsampled Y (B operand) MN-major: rows of the Y tiles are K, samples are contiguous
+    constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N) | IDESC_B_MN_MAJOR, idesc8 = idesc_f8_f32(TILE_M, TILE_N) | IDESC_B_MN_MAJOR;
     constexpr uint32_t T16 = RTILE_BYTES >> 4;                    // operand tile size in 16-byte descriptor units
+    constexpr uint32_t YK16 = 2048 >> 4, YK8 = 4096 >> 4;          // one MMA of K: 16 fp16 rows / 32 byte rows of 128 B
     int stage = 0; uint32_t phase = 0; int it = 0;
     const uint64_t ring_d = desc_kmajor_sw(smem_u32(ring), RBK), res_d = desc_kmajor_sw(smem_u32(smem), RBK);
+    const uint64_t ring_y16 = desc_mnmajor_sw128(smem_u32(ring), RTILE_BYTES / 2), ring_y8 = desc_mnmajor_sw128(smem_u32(ring), 16);
     for (int ti = i_begin; ti < i_end; ++ti) {
       const TcReconTile tl = tiles[ti];
       const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + RBK - 1) / RBK;
@@ -171,6 +179,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           tc_fence_after_sync();
           // base descriptors; every operand tile / K step is a constant added to the 16-byte address field
           const uint64_t sd = ring_d + (uint64_t)(stage * (STAGE_BYTES >> 4));
+          const uint64_t sy16 = ring_y16 + (uint64_t)(stage * (STAGE_BYTES >> 4)), sy8 = ring_y8 + (uint64_t)(stage * (STAGE_BYTES >> 4));
           const uint64_t rd = RES ? res_d + (uint64_t)(kb * 4 * T16) : sd;
           const int nk = min(RBK / 16, (Kpad - kb * RBK) / 16);    // K is padded to 16: the last box may be partly zero fill
           if (elect_one()) {
@@ -179,19 +188,19 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
               if (k >= nk) break;
               const bool acc = (kb | k) != 0;
               if (RES) {
-                const uint64_t y_hi = sd + 2 * k, y_8 = sd + (T16 + 2 * k);
+                const uint64_t y_hi = sy16 + YK16 * k, y_8 = sy8 + (T16 + YK8 * k);
                 mma_f16_ss(d_re, rd + (0 * T16 + 2 * k), y_hi, idesc, acc);
                 mma_f16_ss(d_im, rd + (1 * T16 + 2 * k), y_hi, idesc, acc);
                 mma_f8_ss(d_re, rd + (2 * T16 + 2 * k), y_8, idesc8, true);
                 mma_f8_ss(d_im, rd + (3 * T16 + 2 * k), y_8, idesc8, true);
               } else {
-                const uint64_t y_hi = sd + (2 * T16 + 2 * k);
+                const uint64_t y_hi = sy16 + (2 * T16 + YK16 * k);
                 mma_f16_ss(d_re, sd + (0 * T16 + 2 * k), y_hi, idesc, acc);
                 mma_f16_ss(d_im, sd + (1 * T16 + 2 * k), y_hi, idesc, acc);
                 if (PLANES == 2) {
                   // the correction planes: 32 bytes = 16 of K as (e4m3, e4m3) x (e5m2, e5m2) pairs -> one fp8 MMA adds
                   // both cross terms R_hi Y_lo + R_lo Y_hi
-                  const uint64_t y_8 = sd + (5 * T16 + 2 * k);
+                  const uint64_t y_8 = sy8 + (5 * T16 + YK8 * k);
                   mma_f8_ss(d_re, sd + (3 * T16 + 2 * k), y_8, idesc8, true);
                   mma_f8_ss(d_im, sd + (4 * T16 + 2 * k), y_8, idesc8, true);
                 }
@@ -712,6 +721,22 @@ static bool make_map(CUtensorMap *m, const void *base, uint64_t rows, uint64_t c
   return true;
 }
 
+// upsampled-Y planes: rows of `cols` elements (fp16: bytes = false, correction plane: bytes = true), boxes of 128 B x box_rows, 128-byte swizzle
+static bool make_map_y(CUtensorMap *m, const void *base, bool bytes, uint64_t rows, uint64_t cols, int box_rows) {
+  EncodeTiledFn enc = get_encode();
+  if (!enc) { set_error("stream_create: cuTensorMapEncodeTiled is not available from the driver"); return false; }
+  cuuint64_t dims[2] = {cols, rows};
+  cuuint64_t strides[1] = {cols * (bytes ? 1 : 2)};
+  cuuint32_t box[2] = {(cuuint32_t)(bytes ? 128 : 64), (cuuint32_t)box_rows};
+  cuuint32_t estr[2] = {1, 1};
+  CUresult r = enc(m, bytes ? CU_TENSOR_MAP_DATA_TYPE_UINT8 : CU_TENSOR_MAP_DATA_TYPE_FLOAT16, 2, const_cast<void *>(base), dims, strides, box, estr,
+                   CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B, CU_TENSOR_MAP_L2_PROMOTION_L2_256B,
+                   CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) { set_error("stream_create: cuTensorMapEncodeTiled failed (%d) for the upsampled-Y plane [%llu][%llu]", (int)r,
+                                     (unsigned long long)rows, (unsigned long long)cols); return false; }
+  return true;
+}
+
 template <typename T>
 static bool plan_upload(TcPlan *p, T **dst, const std::vector<T> &h) {
   void *q = nullptr;
@@ -792,13 +817,23 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   for (size_t b = 0; b < banks.size(); ++b) {
     const ReconBank &k = banks[b];
     memset(&rb[b], 0, sizeof(TcReconBank));
+    const uint64_t Bp = (uint64_t)yup_pitch(B), yrows = (uint64_t)n_det * k.Kpad;
+    const uint8_t *y8 = reinterpret_cast<const uint8_t *>(k.yup) + 2 * k.yup_plane_stride;      // the correction plane (bytes)
     if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_RES) ||
-        !make_map(&rb[b].mapY, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK_RES) ||
         !make_map(&rb[b].mapR64, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_STR) ||
-        !make_map(&rb[b].mapY64, k.yup, (uint64_t)planes * n_det * B, (uint64_t)k.Kpad, TILE_M, RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+        !make_map_y(&rb[b].mapY, k.yup, false, yrows, Bp, RBK_RES) || !make_map_y(&rb[b].mapY64, k.yup, false, yrows, Bp, RBK_STR)) {
+      tc_plan_destroy(p); return LLOID_ECUDA;
+    }
+    if (planes == 2 && (!make_map_y(&rb[b].mapY8, y8, true, 2 * yrows, Bp, 2 * RBK_RES) || !make_map_y(&rb[b].mapY8_64, y8, true, 2 * yrows, Bp, 2 * RBK_STR))) {
+      tc_plan_destroy(p); return LLOID_ECUDA;
+    }
     rb[b].M = k.M; rb[b].Mpad = k.Mpad; rb[b].Kpad = k.Kpad; rb[b].tmpl_off = k.tmpl_off; rb[b].inv_scale = k.inv_scale;
     rb[b].acorr = k.acorr; rb[b].xi_delta = k.xi_delta;
-    if (xi_delta > 0 && !make_map(&rb[b].mapYh, k.yhist, (uint64_t)planes * n_det * 3 * B, (uint64_t)k.Kpad, TILE_M, RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    if (xi_delta > 0) {                                        // history ring: rows of 3 B samples, plane stride n_det * Kpad * 3 B
+      const uint8_t *h8 = reinterpret_cast<const uint8_t *>(k.yhist) + 2 * yrows * 3 * (uint64_t)B;
+      if (!make_map_y(&rb[b].mapYh, k.yhist, false, yrows, 3 * (uint64_t)B, RBK_STR) ||
+          !make_map_y(&rb[b].mapYh8, h8, true, 2 * yrows, 3 * (uint64_t)B, 2 * RBK_STR)) { tc_plan_destroy(p); return LLOID_ECUDA; }
+    }
     // resident R pays when the item reuses it over enough tiles (short buffers, config 4, stream R with Y instead)
     is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && (long long)n_det * ((B + TILE_N - 1) / TILE_N) >= 8) ? 1 : 0;
     const long long mt = (k.M + TILE_M - 1) / TILE_M;

@@ -88,9 +88,10 @@ struct UpRow {                       // one basis row of one slice of one bank: 
   const float *ysrc;                 // class Y ring + stacked row index (detector 0, segment 0)
   long long ydet_stride, yseg_stride;
   void *yup;                         // bank's upsampled-Y array (plane 0)
-  long long dst0;                    // element offset of (detector 0, sample 0, this row's column)
+  long long dst0;                    // element offset of (detector 0, sample 0) of this row: its column (FFMA) / column * yup_pitch(B)
   long long yup_det_stride, yup_plane_stride;
-  int nseg, ypitch, kpitch, bank;    // bank: index of the owning bank (items are ordered by it for L2 locality)
+  int nseg, ypitch, kpitch, bank;    // kpitch: Kpad (FFMA, sample pitch) / yup_pitch(B) (tensor-core layouts, row pitch);
+                                     // bank: index of the owning bank (items are ordered by it for L2 locality)
 };
 struct UpItem {                      // <= 32 rows (lanes) that share one upsample chain: (rate, stage factors)
   int row0, nl;                      // rows [row0, row0 + nl) of the UpRow table
@@ -99,11 +100,15 @@ struct UpItem {                      // <= 32 rows (lanes) that share one upsamp
   int ylen;                          // Y ring length at this rate (B/D + 32)
 };
 
+// Tensor-core modes: the upsampled-Y planes hold one row of yup_pitch(B) samples per (detector, basis row) -- sample-contiguous,
+// so that the upsampler stores whole 32-byte sectors and a3 reads them as an MN-major operand
+inline int yup_pitch(int B) { return (B + 63) & ~63; }
+
 struct ReconBank {                   // a3 work description of one bank
   const float *R32; const __half *R16; long long r_part_stride, r_plane_stride;
   const void *yup; long long yup_det_stride, yup_plane_stride;
   int M, Mpad, Kpad, tmpl_off;       // tmpl_off: first template of this bank in the stream's peak array
-  const void *yhist;                 // xi^2: [planes][n_det][3 B][Kpad] ring of the last three pushes' upsampled Y (or nullptr)
+  const void *yhist;                 // xi^2: [planes][n_det][Kpad (x2 byte rows in plane 1)][3 B] ring of the last three pushes' upsampled Y (or nullptr)
   const float2 *acorr; int xi_delta; // xi^2: the bank's autocorrelations
   float inv_scale2;                  // 1/(r_scale^2): applied to |z|^2
   float inv_scale;
@@ -121,7 +126,8 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
                             const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st);
 cudaError_t launch_recon_ffma(const ReconBank *banks_dev, int n_banks, int max_mtiles, int n_det, int B,
                               PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st);
-struct YupCopy { const uint4 *src; uint4 *dst; long long n16; long long dst_slot_stride16; };   // one (bank, plane, detector) piece
+// one (bank, plane, detector) piece: n_rows rows of row16 16-byte units (B samples), contiguous in the source, dst_pitch16 apart in the ring
+struct YupCopy { const uint4 *src; uint4 *dst; long long n_rows, row16, dst_pitch16; };
 cudaError_t launch_yup_copy(const YupCopy *table_dev, int n_pieces, int slot, cudaStream_t st);
 cudaError_t launch_xi2_finalize(const float *xi_partial, const lloid_peak *peaks, const float *den, int n_det, int Mtot, float *xi2_out,
                                 cudaStream_t st);

@@ -297,24 +297,28 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   for (int b = 0; b < n_banks; ++b) {
     const lloid_bank *bk = s->banks[b];
     ReconBank rb; memset(&rb, 0, sizeof(rb));
-    size_t plane_elems = (size_t)n_det * B * bk->Kpad;
+    // FFMA: fp32 [n_det][B][Kpad]; tensor-core modes: [planes][n_det][Kpad][Bp] 16-bit units, sample-contiguous rows
+    const int Bp = s->up_planes == 0 ? B : yup_pitch(B);
+    size_t plane_elems = (size_t)n_det * Bp * bk->Kpad;
     void *yup = nullptr;
     if (s->up_planes == 0) { float *p; CK(dev_alloc(s, &p, plane_elems)); yup = p; }
     else { __half *p; CK(dev_alloc(s, &p, plane_elems * planes)); yup = p; }
     if (s->xi_delta > 0) {
       __half *h; CK(dev_alloc(s, &h, plane_elems * planes * 3, true));        // zero = "before the stream started"
       rb.yhist = h; rb.acorr = bk->dAcorr; rb.xi_delta = bk->xi_delta;
-      for (int pd = 0; pd < planes * n_det; ++pd) {
+      for (int pd = 0; pd < planes * n_det; ++pd) {             // B % 128 == 0 here, so Bp == B: the rows of a piece are contiguous
         YupCopy c;
         c.src = reinterpret_cast<const uint4 *>((const __half *)yup + (size_t)pd * B * bk->Kpad);
         c.dst = reinterpret_cast<uint4 *>(h + (size_t)pd * 3 * B * bk->Kpad);
-        c.n16 = (long long)B * bk->Kpad * 2 / 16; c.dst_slot_stride16 = c.n16;
+        const bool byte_rows = pd >= n_det;                     // plane 1: two rows of B bytes per basis row
+        c.n_rows = byte_rows ? 2 * bk->Kpad : bk->Kpad;
+        c.row16 = (byte_rows ? B : 2 * B) / 16; c.dst_pitch16 = 3 * c.row16;
         ycopies.push_back(c);
       }
     }
     rb.R32 = bk->dR32; rb.R16 = bk->dR16;
     rb.r_part_stride = (long long)bk->Mpad * bk->Kpad; rb.r_plane_stride = 2 * rb.r_part_stride;
-    rb.yup = yup; rb.yup_det_stride = (long long)B * bk->Kpad; rb.yup_plane_stride = (long long)plane_elems;
+    rb.yup = yup; rb.yup_det_stride = (long long)Bp * bk->Kpad; rb.yup_plane_stride = (long long)plane_elems;
     rb.M = bk->M; rb.Mpad = bk->Mpad; rb.Kpad = bk->Kpad; rb.tmpl_off = s->Mtot;
     rb.inv_scale = 1.f / bk->r_scale; rb.inv_scale2 = rb.inv_scale * rb.inv_scale;
     s->rbanks.push_back(rb);
@@ -334,8 +338,10 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
         UpRow r; memset(&r, 0, sizeof(r));
         r.ysrc = cc.yring + row_off[b][i] + l; r.ydet_stride = cc.ydet_stride; r.yseg_stride = cc.yseg_stride;
         r.nseg = cc.nseg; r.ypitch = cc.Lpad;
-        r.yup = yup; r.dst0 = si.koff + l; r.yup_det_stride = rb.yup_det_stride; r.yup_plane_stride = rb.yup_plane_stride;
-        r.kpitch = bk->Kpad; r.bank = b;
+        r.yup = yup; r.yup_det_stride = rb.yup_det_stride; r.yup_plane_stride = rb.yup_plane_stride;
+        if (s->up_planes == 0) { r.dst0 = si.koff + l; r.kpitch = bk->Kpad; }
+        else { r.dst0 = (long long)(si.koff + l) * Bp; r.kpitch = Bp; }
+        r.bank = b;
         dst.push_back(r);
       }
       rate_sum += (double)si.L * si.rate;

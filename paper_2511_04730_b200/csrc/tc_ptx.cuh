@@ -119,6 +119,15 @@ __device__ __forceinline__ uint64_t desc_kmajor_nosw(uint32_t smem_addr, uint32_
   return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(sbo_bytes >> 4) << 32) |
          ((uint64_t)1 << 46);
 }
+// MN-major operand, 128-byte swizzle (the upsampled-Y operand of a3: rows = K, 128 contiguous bytes along N per row as a TMA
+// box with the 128-byte swizzle writes them): 8 K rows = one 1024-byte atom, SBO = byte stride between 8-row groups along K,
+// LBO = byte stride between 128-byte blocks along N (64 fp16 / 128 fp8 elements).  Advancing K by one MMA = +16 rows
+// (fp16, 2048 B) / +32 rows (fp8, 4096 B) on the start address.  Needs the b_major bit (16) of the instruction descriptor.
+__device__ __forceinline__ uint64_t desc_mnmajor_sw128(uint32_t smem_addr, uint32_t lbo_bytes) {
+  return (uint64_t)((smem_addr & 0x3FFFF) >> 4) | ((uint64_t)(lbo_bytes >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | ((uint64_t)1 << 46) |
+         ((uint64_t)2 << 61);
+}
+static constexpr uint32_t IDESC_B_MN_MAJOR = 1u << 16;
 // kind::f16 instruction descriptor: D = fp32, A = B = fp16, both K-major, no negate, dense.
 __host__ __device__ constexpr uint32_t idesc_f16_f32(int M, int N) {
   return (1u << 4) | ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
