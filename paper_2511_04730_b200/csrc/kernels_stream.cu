@@ -141,12 +141,16 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 #define UP_RUN 8
 #define UP_LD 8      // ring columns loaded per round and warp
 #define UP_CHUNK 512  // f0 samples per CTA
-#define UP_MAXW (UP_CHUNK / 2 + 40)   // widest staged level: chunk/2 + 2*8 + 1 (+ slack)
-#define UP_TT 256                     // samples per output tile (tensor-core layouts)
+// Staged levels: w_h <= (w_{h-1} - 1) / f + 18, f >= 2, so level 1 has <= chunk/2 + 17 columns and level 2 <= 154 (chunk
+// 512).  Odd levels live in buffer A, even ones and the output tile in the smaller buffer B: 55 KB, four CTAs per SM.
+#define UP_WA (UP_CHUNK / 2 + 20)
+#define UP_WB (UP_CHUNK / 4 + 28)
+#define UP_SMEM ((UP_WA + UP_WB) * 32 * 4)
+#define UP_TT 128                     // samples per output tile (tensor-core layouts)
 #define UP_P16 (UP_TT * 2 + 16)       // tile row pitches in bytes: odd multiples of 16, so 16-byte accesses by lane = row do not conflict
 #define UP_P8 (UP_TT + 16)
 #define UP_T8 (32 * UP_P16)           // byte rows start here: row = term * 32 + lane
-static_assert(UP_T8 + 64 * UP_P8 <= UP_MAXW * 32 * 4, "the output tile must fit one staging buffer");
+static_assert(UP_T8 + 64 * UP_P8 <= UP_WB * 32 * 4, "the output tile must fit staging buffer B");
 
 // the two correction bytes of DESIGN.md section 4 for a value v whose fp16 rounding is hf: e5m2(4 (v - hf)), e5m2(hf / 256)
 __device__ __forceinline__ unsigned short up_pair_lo(float v0, float h0, float v1, float h1) {
@@ -193,13 +197,13 @@ __device__ __forceinline__ void tile_put8(unsigned char *tile, int lane, int tc,
 __device__ __forceinline__ void up_store_f32(void *yup, size_t o, float v) { reinterpret_cast<float *>(yup)[o] = v; }
 
 template <int HALF_PLANES>
-__global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
+__global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
                                                           const float *__restrict__ uptaps,
                                                           const int *__restrict__ uptap_off,
                                                           const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
   static_assert(UP_LD == 8, "tile_put8 takes the UP_LD columns of one load round");
   extern __shared__ __align__(16) float up_dyn[];
-  float(*buf)[UP_MAXW][32] = reinterpret_cast<float(*)[UP_MAXW][32]>(up_dyn);
+  float(*bufA)[32] = reinterpret_cast<float(*)[32]>(up_dyn), (*bufB)[32] = bufA + UP_WA;    // level h: A if h is odd, else B
   __shared__ int s_r0[LLOID_MAX_GROUPS + 1], s_w[LLOID_MAX_GROUPS + 1], s_lf[LLOID_MAX_GROUPS + 1], s_slot0;
   __shared__ unsigned char *s_dst16[32], *s_dst8[32];     // tensor-core layouts: where sample ka of each lane's row goes
   const UpItem *it = &items[blockIdx.y];
@@ -265,10 +269,11 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
         for (int i = 0; i < UP_LD; ++i) v[i] += t[i][j];
     }
   };
-  // tile -> global: 16-byte vectors, a warp instruction covers 256 samples of one fp16 row / 2 x 256 of two byte rows
+  // tile -> global: 16-byte vectors, a warp instruction covers UP_TT samples of 32 / (UP_TT / 8) fp16 rows or twice as many byte rows
   auto flush = [&](const unsigned char *tile, int c_lo, int ncol) {
-    for (int r = warp; r < nl; r += nwarp) {
-      const int tc = lane * 8;
+    constexpr int L16 = UP_TT / 8, L8 = UP_TT / 16;          // lanes per row
+    for (int r = warp * (32 / L16) + lane / L16; r < nl; r += nwarp * (32 / L16)) {
+      const int tc = (lane % L16) * 8;
       unsigned char *dst = s_dst16[r] + 2 * (c_lo + tc);
       const unsigned char *src = tile + r * UP_P16 + 2 * tc;
       if (tc + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
@@ -277,8 +282,8 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
           if (tc + j < ncol) reinterpret_cast<unsigned short *>(dst)[j] = reinterpret_cast<const unsigned short *>(src)[j];
     }
     if (HALF_PLANES == 2) {
-      for (int rr = 2 * warp + (lane >> 4); rr < 64; rr += 2 * nwarp) {      // rr = term * 32 + row
-        const int r = rr & 31, tc = (lane & 15) * 16;
+      for (int rr = warp * (32 / L8) + lane / L8; rr < 64; rr += nwarp * (32 / L8)) {      // rr = term * 32 + row
+        const int r = rr & 31, tc = (lane % L8) * 16;
         if (r < nl) {
           unsigned char *dst = s_dst8[r] + (size_t)(rr >> 5) * kpitch + c_lo + tc;
           const unsigned char *src = tile + UP_T8 + rr * UP_P8 + tc;
@@ -302,7 +307,7 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
           if (active && c0 + i < w0) up_store_f32(yup, out0 + (size_t)(c0 + i) * kpitch, v[i]);
       }
     } else {
-      unsigned char *tile = reinterpret_cast<unsigned char *>(buf[0]);
+      unsigned char *tile = reinterpret_cast<unsigned char *>(bufB);
       for (int c_lo = 0; c_lo < w0; c_lo += UP_TT) {
         const int c_hi = min(c_lo + UP_TT, w0);
         for (int c0 = c_lo + warp * UP_LD; c0 < c_hi; c0 += UP_LD * nwarp) {
@@ -325,12 +330,13 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
 
   // level G from the Y ring
   const int wg = s_w[G];
+  float(*lvG)[32] = (G & 1) ? bufA : bufB;
   for (int c0 = warp * UP_LD; c0 < wg; c0 += UP_LD * nwarp) {
     float v[UP_LD];
     load_yn(c0, wg, v);
 #pragma unroll
     for (int i = 0; i < UP_LD; ++i)
-      if (c0 + i < wg) buf[0][c0 + i][lane] = v[i];
+      if (c0 + i < wg) lvG[c0 + i][lane] = v[i];
   }
   __syncthreads();
   // The run of one warp: UP_RUN consecutive inputs qq = q0 + u of a stage, held in registers with their 15 neighbours:
@@ -352,7 +358,6 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
     odd[u] = v0 + v1;                                                                              \
   }
 
-  int cur = 0;
   for (int h = G; h >= 2; --h) {                             // stages that stay in shared memory
     const int lf = s_lf[h], f = 1 << lf, r0 = s_r0[h], wout = s_w[h - 1];
     // Output c (relative to lo_{h-1}) has input index qq = (r0 + c) >> lf relative to floor(lo_{h-1}/f) and phase
@@ -360,8 +365,8 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
     // last warp's last run is ragged).
     const int nq = ((r0 + wout - 1) >> lf) + 1, per = ((nq + nwarp - 1) / nwarp + UP_RUN - 1) / UP_RUN * UP_RUN;
     const int qa = warp * per, qb = min(qa + per, nq);
-    const float(*in)[32] = buf[cur];
-    float(*out)[32] = buf[cur ^ 1];
+    const float(*in)[32] = (h & 1) ? bufA : bufB;
+    float(*out)[32] = (h & 1) ? bufB : bufA;
     for (int q0 = qa; q0 < qb; q0 += UP_RUN) {
       UP_LOAD_RUN()
       if (f == 2) {
@@ -405,15 +410,14 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
       }
     }
     __syncthreads();
-    cur ^= 1;
   }
 
   // last stage (to f0).  FFMA mode stores every output directly; the tensor-core layouts go through the tile, UP_TT output
   // samples at a time (the staging buffer not read by this stage), every warp taking its share of each tile's runs.
   {
     const int lf = s_lf[1], f = 1 << lf, r0 = s_r0[1], wout = s_w[0];
-    const float(*in)[32] = buf[cur];
-    unsigned char *tile = reinterpret_cast<unsigned char *>(buf[cur ^ 1]);
+    const float(*in)[32] = bufA;
+    unsigned char *tile = reinterpret_cast<unsigned char *>(bufB);
     const float *g = uptaps + uptap_off[lf];
     const int tt = HALF_PLANES == 0 ? wout : UP_TT;
     for (int c_lo = 0; c_lo < wout; c_lo += tt) {
@@ -493,7 +497,7 @@ __global__ void __launch_bounds__(256, 3) upsample_kernel(const UpItem *__restri
 // Per-device kernel attributes (dynamic shared memory opt-in) and the x2 taps: called by every lloid_stream_create on
 // its current device (the attribute is per device/context, not per process).
 cudaError_t upsample_configure(UpTaps2 *t2) {
-  const int smem = 2 * UP_MAXW * 32 * (int)sizeof(float);
+  const int smem = UP_SMEM;
   cudaError_t e = cudaFuncSetAttribute(upsample_kernel<0>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(upsample_kernel<1>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
   if (e == cudaSuccess) e = cudaFuncSetAttribute(upsample_kernel<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem);
@@ -507,7 +511,7 @@ cudaError_t upsample_configure(UpTaps2 *t2) {
 cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int n_items, int n_det, int B, int chunk, const float *uptaps,
                             const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
-  const int smem = 2 * UP_MAXW * 32 * (int)sizeof(float);
+  const int smem = UP_SMEM;
   if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   else upsample_kernel<2><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
