@@ -247,22 +247,24 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
   // parallelism is what the load phase needs); the split-K partial sums are then added in segment order (deterministic,
   // the same order for every caller).  Columns never computed at stream start are the ring's zeros.
   auto load_yn = [&](int c0, int c_end, float (&v)[UP_LD]) {
-    int sl[UP_LD];
-    bool ok[UP_LD];
+    unsigned off[UP_LD];                                      // element offsets inside one (segment, detector) ring: < 2^31 (checked at create)
     const int slot = (s_slot0 + c0) % ylen;
+    const int nok = active ? min(UP_LD, c_end - c0) : 0;      // columns [c0, c0 + nok) exist
 #pragma unroll
     for (int i = 0; i < UP_LD; ++i) {
-      sl[i] = slot + i >= ylen ? slot + i - ylen : slot + i;
-      ok[i] = active && c0 + i < c_end;
+      const int sl = slot + i >= ylen ? slot + i - ylen : slot + i;
+      off[i] = (unsigned)sl * (unsigned)ypitch;
       v[i] = 0.f;
     }
-    for (int sg0 = 0; sg0 < nseg; sg0 += 2) {
+    const float *ys = yr;
+    for (int sg0 = 0; sg0 < nseg; sg0 += 2, ys += 2 * yseg) {
+      const float *ys1 = ys + yseg;
+      const int nok1 = sg0 + 1 < nseg ? nok : 0;
       float t[UP_LD][2];
 #pragma unroll
-      for (int j = 0; j < 2; ++j)
+      for (int i = 0; i < UP_LD; ++i) t[i][0] = i < nok ? __ldg(ys + off[i]) : 0.f;
 #pragma unroll
-        for (int i = 0; i < UP_LD; ++i)
-          t[i][j] = (ok[i] && sg0 + j < nseg) ? __ldg(yr + (size_t)(sg0 + j) * yseg + (size_t)sl[i] * ypitch) : 0.f;
+      for (int i = 0; i < UP_LD; ++i) t[i][1] = i < nok1 ? __ldg(ys1 + off[i]) : 0.f;
 #pragma unroll
       for (int j = 0; j < 2; ++j)
 #pragma unroll
@@ -272,11 +274,12 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
   // tile -> global: 16-byte vectors, a warp instruction covers UP_TT samples of 32 / (UP_TT / 8) fp16 rows or twice as many byte rows
   auto flush = [&](const unsigned char *tile, int c_lo, int ncol) {
     constexpr int L16 = UP_TT / 8, L8 = UP_TT / 16;          // lanes per row
+    const bool whole = ncol == UP_TT;                        // (a ragged tile: buffer_len not a multiple of UP_TT)
     for (int r = warp * (32 / L16) + lane / L16; r < nl; r += nwarp * (32 / L16)) {
       const int tc = (lane % L16) * 8;
       unsigned char *dst = s_dst16[r] + 2 * (c_lo + tc);
       const unsigned char *src = tile + r * UP_P16 + 2 * tc;
-      if (tc + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+      if (whole || tc + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
       else
         for (int j = 0; j < 8; ++j)
           if (tc + j < ncol) reinterpret_cast<unsigned short *>(dst)[j] = reinterpret_cast<const unsigned short *>(src)[j];
@@ -287,7 +290,7 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
         if (r < nl) {
           unsigned char *dst = s_dst8[r] + (size_t)(rr >> 5) * kpitch + c_lo + tc;
           const unsigned char *src = tile + UP_T8 + rr * UP_P8 + tc;
-          if (tc + 16 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+          if (whole || tc + 16 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
           else
             for (int j = 0; j < 16; ++j)
               if (tc + j < ncol) dst[j] = src[j];
@@ -345,7 +348,11 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
 #define UP_LOAD_RUN()                                                                              \
   const int nrun = min(UP_RUN, qb - q0);                                                           \
   float X[UP_RUN + 15];                                                                            \
-  _Pragma("unroll") for (int j = 0; j < UP_RUN + 15; ++j) X[j] = (j < nrun + 15) ? in[q0 + 1 + j][lane] : 0.f; \
+  if (nrun == UP_RUN) {                                     /* warp-uniform: no per-element predicate */   \
+    _Pragma("unroll") for (int j = 0; j < UP_RUN + 15; ++j) X[j] = in[q0 + 1 + j][lane];           \
+  } else {                                                                                         \
+    _Pragma("unroll") for (int j = 0; j < UP_RUN + 15; ++j) X[j] = (j < nrun + 15) ? in[q0 + 1 + j][lane] : 0.f; \
+  }                                                                                                \
   const int cbase = (q0 << lf) - r0;                        /* output index of (u = 0, phase 0) */
 #define UP_ODD_X2()                                                                                \
   float odd[UP_RUN];                                                                               \

@@ -260,6 +260,10 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
       __half *p; CK(dev_upload(s, &p, U16)); cc.U16 = p;
     }
     cc.nseg = (s->precision == LLOID_PREC_FP32_FFMA) ? 1 : tc_k_segments(cc.Npad);
+    if ((size_t)cc.ylen * cc.Lpad >= ((size_t)1 << 31)) {       // the upsampler addresses a ring with 32-bit element offsets
+      set_error("stream_create: a basis-output ring of %d columns x %d rows exceeds 2^31 elements; use fewer banks per stream", cc.ylen, cc.Lpad);
+      lloid_stream_destroy(s); return LLOID_EINVAL;
+    }
     CK(dev_alloc(s, &cc.yring, (size_t)cc.nseg * n_det * cc.ylen * cc.Lpad, true));
     cc.ydet_stride = (long long)cc.ylen * cc.Lpad;
     cc.yseg_stride = (long long)n_det * cc.ydet_stride;
