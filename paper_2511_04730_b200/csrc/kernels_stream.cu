@@ -138,6 +138,7 @@ cudaError_t launch_decimate(const DecimParams &P, const float *strain, const lon
 //   samples of a row are contiguous and the CTA stages UP_TT samples x 32 rows in shared memory, then writes them with
 //   16-byte vectors, whole sectors only.  FFMA mode (HALF_PLANES 0) keeps fp32 [sample][Kpad] and stores directly.
 // ------------------------------------------------------------------------------------------------
+#define UP_THREADS 256
 #define UP_RUN 8
 #define UP_LD 8      // ring columns loaded per round and warp
 #define UP_CHUNK 512  // f0 samples per CTA
@@ -197,7 +198,7 @@ __device__ __forceinline__ void tile_put8(unsigned char *tile, int lane, int tc,
 __device__ __forceinline__ void up_store_f32(void *yup, size_t o, float v) { reinterpret_cast<float *>(yup)[o] = v; }
 
 template <int HALF_PLANES>
-__global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
+__global__ void __launch_bounds__(UP_THREADS, HALF_PLANES == 0 ? 3 : 4) upsample_kernel(const UpItem *__restrict__ items, const UpRow *__restrict__ rows, int B, int chunk,
                                                           const float *__restrict__ uptaps,
                                                           const int *__restrict__ uptap_off,
                                                           const long long *__restrict__ n0_ptr, const UpTaps2 taps2) {
@@ -210,7 +211,8 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
   const int det = blockIdx.z;
   const int ka = blockIdx.x * chunk;
   const int kb = min(ka + chunk, B);
-  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5, nwarp = blockDim.x >> 5;
+  constexpr int nwarp = UP_THREADS / 32;                       // compile-time: the run partition divides by it
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int G = it->g, nl = it->nl;
   const bool active = lane < nl;
   const UpRow *rw = &rows[it->row0 + (active ? lane : 0)];     // this lane's row: source ring row and destination
@@ -259,12 +261,19 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
     const float *ys = yr;
     for (int sg0 = 0; sg0 < nseg; sg0 += 2, ys += 2 * yseg) {
       const float *ys1 = ys + yseg;
-      const int nok1 = sg0 + 1 < nseg ? nok : 0;
       float t[UP_LD][2];
+      if (nok == UP_LD && sg0 + 1 < nseg) {                   // the common case: no per-load predicate
 #pragma unroll
-      for (int i = 0; i < UP_LD; ++i) t[i][0] = i < nok ? __ldg(ys + off[i]) : 0.f;
+        for (int i = 0; i < UP_LD; ++i) t[i][0] = __ldg(ys + off[i]);
 #pragma unroll
-      for (int i = 0; i < UP_LD; ++i) t[i][1] = i < nok1 ? __ldg(ys1 + off[i]) : 0.f;
+        for (int i = 0; i < UP_LD; ++i) t[i][1] = __ldg(ys1 + off[i]);
+      } else {
+        const int nok1 = sg0 + 1 < nseg ? nok : 0;
+#pragma unroll
+        for (int i = 0; i < UP_LD; ++i) t[i][0] = i < nok ? __ldg(ys + off[i]) : 0.f;
+#pragma unroll
+        for (int i = 0; i < UP_LD; ++i) t[i][1] = i < nok1 ? __ldg(ys1 + off[i]) : 0.f;
+      }
 #pragma unroll
       for (int j = 0; j < 2; ++j)
 #pragma unroll
@@ -274,26 +283,33 @@ __global__ void __launch_bounds__(256, HALF_PLANES == 0 ? 3 : 4) upsample_kernel
   // tile -> global: 16-byte vectors, a warp instruction covers UP_TT samples of 32 / (UP_TT / 8) fp16 rows or twice as many byte rows
   auto flush = [&](const unsigned char *tile, int c_lo, int ncol) {
     constexpr int L16 = UP_TT / 8, L8 = UP_TT / 16;          // lanes per row
+    constexpr int R16 = nwarp * (32 / L16), R8 = nwarp * (32 / L8);   // rows per pass of the CTA
     const bool whole = ncol == UP_TT;                        // (a ragged tile: buffer_len not a multiple of UP_TT)
-    for (int r = warp * (32 / L16) + lane / L16; r < nl; r += nwarp * (32 / L16)) {
-      const int tc = (lane % L16) * 8;
-      unsigned char *dst = s_dst16[r] + 2 * (c_lo + tc);
-      const unsigned char *src = tile + r * UP_P16 + 2 * tc;
-      if (whole || tc + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
-      else
-        for (int j = 0; j < 8; ++j)
-          if (tc + j < ncol) reinterpret_cast<unsigned short *>(dst)[j] = reinterpret_cast<const unsigned short *>(src)[j];
+    const int tc16 = (lane % L16) * 8, tc8 = (lane % L8) * 16;
+#pragma unroll
+    for (int p = 0; p < 32 / R16; ++p) {
+      const int r = p * R16 + warp * (32 / L16) + lane / L16;
+      if (r < nl) {
+        unsigned char *dst = s_dst16[r] + 2 * (c_lo + tc16);
+        const unsigned char *src = tile + r * UP_P16 + 2 * tc16;
+        if (whole || tc16 + 8 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+        else
+          for (int j = 0; j < 8; ++j)
+            if (tc16 + j < ncol) reinterpret_cast<unsigned short *>(dst)[j] = reinterpret_cast<const unsigned short *>(src)[j];
+      }
     }
     if (HALF_PLANES == 2) {
-      for (int rr = warp * (32 / L8) + lane / L8; rr < 64; rr += nwarp * (32 / L8)) {      // rr = term * 32 + row
-        const int r = rr & 31, tc = (lane % L8) * 16;
+#pragma unroll
+      for (int p = 0; p < 64 / R8; ++p) {
+        const int rr = p * R8 + warp * (32 / L8) + lane / L8;                // rr = term * 32 + row
+        const int r = rr & 31;
         if (r < nl) {
-          unsigned char *dst = s_dst8[r] + (size_t)(rr >> 5) * kpitch + c_lo + tc;
-          const unsigned char *src = tile + UP_T8 + rr * UP_P8 + tc;
-          if (whole || tc + 16 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
+          unsigned char *dst = s_dst8[r] + (size_t)(rr >> 5) * kpitch + c_lo + tc8;
+          const unsigned char *src = tile + UP_T8 + rr * UP_P8 + tc8;
+          if (whole || tc8 + 16 <= ncol) *reinterpret_cast<uint4 *>(dst) = *reinterpret_cast<const uint4 *>(src);
           else
             for (int j = 0; j < 16; ++j)
-              if (tc + j < ncol) dst[j] = src[j];
+              if (tc8 + j < ncol) dst[j] = src[j];
         }
       }
     }
@@ -519,9 +535,9 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
                             const int *uptap_off, const long long *n0, int out_half_planes, const UpTaps2 &t2, cudaStream_t st) {
   dim3 grid((B + chunk - 1) / chunk, n_items, n_det);
   const int smem = UP_SMEM;
-  if (out_half_planes == 0) upsample_kernel<0><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else if (out_half_planes == 1) upsample_kernel<1><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
-  else upsample_kernel<2><<<grid, 256, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  if (out_half_planes == 0) upsample_kernel<0><<<grid, UP_THREADS, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else if (out_half_planes == 1) upsample_kernel<1><<<grid, UP_THREADS, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
+  else upsample_kernel<2><<<grid, UP_THREADS, smem, st>>>(items_dev, rows_dev, B, chunk, uptaps, uptap_off, n0, t2);
   return cudaGetLastError();
 }
 
