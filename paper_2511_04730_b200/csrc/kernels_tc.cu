@@ -24,7 +24,8 @@ namespace lloid {
 using namespace ptx;
 
 static constexpr int EPI_THREADS = 512;      // a3: 16 epilogue warps
-static constexpr int RECON_THREADS = 64 + EPI_THREADS;   // a3: warps 0 TMA, 1 MMA, 2-17 epilogue
+static constexpr int RECON_THREADS = 64 + EPI_THREADS + 32;   // a3: warps 0 TMA, 1 and 18 MMA (even / odd tiles), 2-17 epilogue
+static constexpr int RECON_MMA2 = RECON_THREADS / 32 - 1;     // the second MMA warp
 static constexpr int PK_CHUNK = 4;           // samples per peak-search chunk
 static constexpr int REC_BYTES = EPI_THREADS * PK_CHUNK * 8;   // saved record chunk (re, im) per epilogue thread: 16 KB
 static constexpr int TILE_M = 128;           // rows of U / templates of R per tile (= UMMA M, TMEM lanes)
@@ -93,9 +94,9 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
 
   if (warp == 0 && lane == 0) {
-    for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
+    for (int i = 0; i < STAGES; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 2); }   // released by both MMA warps
     for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], EPI_THREADS / 32); }
-    mbar_init(rfull, 1); mbar_init(rfree, 1);
+    mbar_init(rfull, 1); mbar_init(rfree, 2);                     // both MMA warps are done with the item's R
     mbar_fence_init();
   }
   if (warp == 1) tmem_alloc(tmem_slot, 512);
@@ -154,10 +155,16 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         }
       }
     }
-  } else if (warp == 1) {
-    // ===== MMA issuer: the whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers),
-    // one elected lane issues the MMAs of a K block and the commits
+  } else if (warp == 1 || warp == RECON_MMA2) {
+    // ===== MMA issuers.  One thread keeps the tensor pipe busy only while it issues an MMA every ~64 cycles (measured: the
+    // pipe queues about one instruction ahead), and each barrier round trip between K blocks or tiles (wait, fence, elect,
+    // commit) is ~300 cycles of one thread's latency.  So TWO warps issue: warp 1 the even tiles of the CTA (TMEM buffer
+    // 0), warp 18 the odd ones (buffer 1) -- every accumulator is still written by one thread in program order (the
+    // result does not depend on timing), and one warp's round trips hide behind the other's MMAs.
+    // The whole warp runs the loops (uniform control flow keeps the descriptors in uniform registers), one elected lane
+    // issues the MMAs of a K block and the commits.
     // R (A operand) is K-major, upsampled Y (B operand) MN-major: rows of the Y tiles are K, samples are contiguous
+    const int par = warp == 1 ? 0 : 1;
     constexpr uint32_t idesc = idesc_f16_f32(TILE_M, TILE_N) | IDESC_B_MN_MAJOR, idesc8 = idesc_f8_f32(TILE_M, TILE_N) | IDESC_B_MN_MAJOR;
     constexpr uint32_t T16 = RTILE_BYTES >> 4;                    // operand tile size in 16-byte descriptor units
     constexpr uint32_t YK16 = 2048 >> 4, YK8 = 4096 >> 4;          // one MMA of K: 16 fp16 rows / 32 byte rows of 128 B
@@ -169,8 +176,22 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
       const int Kpad = banks[tl.bank].Kpad, nkb = (Kpad + RBK - 1) / RBK;
       if (RES) { mbar_wait(rfull, (uint32_t)(ti - i_begin) & 1); tc_fence_after_sync(); }
       const int ntile = tl.ndet * tl.nt;
+      // this warp's last tile of the item (the MMAs that read the item's resident R last), -1: it has none
+      const int my_last = ntile - 1 - ((((it + ntile - 1) & 1) != par) ? 1 : 0);
       for (int tn = 0; tn < ntile; ++tn, ++it) {
-        const int buf = it & 1;
+        if ((it & 1) != par) {
+          // The other warp's tile.  A parity wait is only sound for a waiter that cannot fall two phases behind, so this warp
+          // takes part in the hand-shake of EVERY K block: it waits for the block to land and gives the stage its second
+          // release (empty[] counts two arrivals: the consumer's tcgen05.commit and this one).  The blocks land before this
+          // warp's own next block anyway (the producer loads in tile order), so nothing waits for the observer.
+          for (int kb = 0; kb < nkb; ++kb) {
+            mbar_wait(&full[stage], phase);
+            if (lane == 0) mbar_arrive(&empty[stage]);
+            if (++stage == STAGES) { stage = 0; phase ^= 1; }
+          }
+          continue;
+        }
+        const int buf = par;
         mbar_wait(&tempty[buf], ((it >> 1) & 1) ^ 1);
         tc_fence_after_sync();
         const uint32_t d_re = tmem + buf * 256, d_im = d_re + 128;
@@ -198,8 +219,8 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
                 mma_f16_ss(d_re, sd + (0 * T16 + 2 * k), y_hi, idesc, acc);
                 mma_f16_ss(d_im, sd + (1 * T16 + 2 * k), y_hi, idesc, acc);
                 if (PLANES == 2) {
-                  // the correction planes: 32 bytes = 16 of K as (e4m3, e4m3) x (e5m2, e5m2) pairs -> one fp8 MMA adds
-                  // both cross terms R_hi Y_lo + R_lo Y_hi
+                  // the correction planes: 16 of K as (e4m3, e4m3) pairs of R x two e5m2 byte rows of Y per basis row -> one
+                  // fp8 MMA adds both cross terms R_hi Y_lo + R_lo Y_hi
                   const uint64_t y_8 = sy8 + (5 * T16 + YK8 * k);
                   mma_f8_ss(d_re, sd + (3 * T16 + 2 * k), y_8, idesc8, true);
                   mma_f8_ss(d_im, sd + (4 * T16 + 2 * k), y_8, idesc8, true);
@@ -208,12 +229,13 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
             }
             mma_commit(&empty[stage]);
             if (kb == nkb - 1) mma_commit(&tfull[buf]);
-            if (RES && kb == nkb - 1 && tn == ntile - 1) mma_commit(rfree);
+            if (RES && kb == nkb - 1 && tn == my_last) mma_commit(rfree);
           }
           __syncwarp();
           if (++stage == STAGES) { stage = 0; phase ^= 1; }
         }
       }
+      if (RES && my_last < 0 && lane == 0) mbar_arrive(rfree);      // no tile of this item was ours: nothing of its R is in flight here
     }
   } else {
     // ===== epilogue (16 warps, four per scheduler): thread = one template (TMEM lane) x one 32-sample slice of the tile.
