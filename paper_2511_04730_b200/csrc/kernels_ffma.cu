@@ -167,7 +167,7 @@ __global__ void __launch_bounds__(256) recon_ffma_kernel(const ReconBank *__rest
         if (c.p > best.p) best = c;
       }
       const int n_tt = gridDim.x;
-      partial[((size_t)det * Mtot + bk.tmpl_off + m) * n_tt + blockIdx.x] = best;
+      partial[((size_t)det * n_tt + blockIdx.x) * Mtot + bk.tmpl_off + m] = best;   // [detector][slot][template]
     }
   }
 }

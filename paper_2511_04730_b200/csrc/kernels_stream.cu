@@ -544,47 +544,54 @@ cudaError_t launch_upsample(const UpItem *items_dev, const UpRow *rows_dev, int 
 // ------------------------------------------------------------------------------------------------
 // a5 finalisation: reduce the per-time-tile partial peaks of every template in ascending time order
 // (strict '>' keeps the first maximum), then snr = sqrt(p), phase = atan2(im, re).
-// The last thread also advances the device-side stream clock n0 by B.
+// Thread 0 also advances the device-side stream clock n0 by B.
 // ------------------------------------------------------------------------------------------------
 // With overlapped trigger windows (Fig. 5) the window of a push is [n0 - overlap, n0 + B): `tail` holds, per
 // template, the peak of the PREVIOUS buffer's last `overlap` samples (index relative to that buffer); it competes with
 // the current buffer's peak (being earlier it wins a tie; reported sample = index - B < 0) and is then replaced by the
 // reduction of `tail_partial`, the current buffer's own tail peak.
-__global__ void finalize_kernel(const PeakPartial *__restrict__ partial, int n_det, int Mtot, int n_tt, int g,
+template <int g>
+__global__ void __launch_bounds__(256) finalize_kernel(const PeakPartial *__restrict__ partial, int n_det, int Mtot, int n_tt,
                                 float threshold, lloid_peak *__restrict__ peaks, long long *n0, int B,
                                 PeakPartial *__restrict__ tail, const PeakPartial *__restrict__ tail_partial, int overlap) {
-  // g (power of two <= 32) consecutive lanes share one template: coalesced reads of its n_tt partial peaks, then a
-  // shuffle reduction.  "Better" = larger |z|^2, ties -> lower sample index (= the first maximum in time).
-  const long long gt = (long long)blockIdx.x * blockDim.x + threadIdx.x;
-  if (gt == 0) *n0 += B;
-  const long long t = gt / g;
-  const int li = (int)(gt % g);
+  // The partial peaks are laid out [detector][slot][template]: for one slot the threads of a warp read consecutive
+  // templates (coalesced 16-byte loads).  A block takes 256 / g (detector, template) pairs; thread (li, jj) reduces the slots
+  // li, li + g, ... of pair jj, the g results meet in shared memory (g = 1 when there are enough pairs to fill the GPU).
+  // "Better" = larger |z|^2, ties -> lower sample index (= the first maximum in time), so the order of the reduction is free.
+  __shared__ PeakPartial red[g > 1 ? 256 : 1];
+  constexpr int tpb = 256 / g;
+  const int li = threadIdx.x / tpb, jj = threadIdx.x - li * tpb;
+  const long long t = (long long)blockIdx.x * tpb + jj;
+  if (blockIdx.x == 0 && threadIdx.x == 0) *n0 += B;
   const bool valid = t < (long long)n_det * Mtot;
+  const int det = valid ? (int)(t / Mtot) : 0, j = valid ? (int)(t - (long long)det * Mtot) : 0;
   PeakPartial best;
   best.p = -2.f; best.idx = 0x7fffffff; best.re = 0.f; best.im = 0.f;
   if (valid) {
-    const PeakPartial *pp = partial + (size_t)t * n_tt;
+    const PeakPartial *pp = partial + (size_t)det * n_tt * Mtot + j;
+#pragma unroll 4
     for (int i = li; i < n_tt; i += g) {
-      PeakPartial c = pp[i];
+      const PeakPartial c = pp[(size_t)i * Mtot];
       if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
     }
   }
-  for (int o = g >> 1; o > 0; o >>= 1) {
-    PeakPartial c;
-    c.p = __shfl_xor_sync(0xffffffffu, best.p, o);
-    c.idx = __shfl_xor_sync(0xffffffffu, best.idx, o);
-    c.re = __shfl_xor_sync(0xffffffffu, best.re, o);
-    c.im = __shfl_xor_sync(0xffffffffu, best.im, o);
-    if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
+  if (g > 1) {
+    red[threadIdx.x] = best;
+    __syncthreads();
+    if (li != 0) return;
+    for (int i = 1; i < g; ++i) {
+      const PeakPartial c = red[i * tpb + jj];
+      if (c.p > best.p || (c.p == best.p && c.idx < best.idx)) best = c;
+    }
   }
-  if (!valid || li != 0) return;
+  if (!valid) return;
   if (tail != nullptr) {
     const PeakPartial tp = tail[t];
     if (tp.idx >= B - overlap && tp.idx < B && tp.p >= best.p) { best = tp; best.idx = tp.idx - B; }
     PeakPartial nt;
     nt.p = -3.f; nt.idx = 0x7fffffff; nt.re = 0.f; nt.im = 0.f;
     for (int i = 0; i < 4; ++i) {
-      const PeakPartial c = tail_partial[(size_t)t * 4 + i];
+      const PeakPartial c = tail_partial[((size_t)det * 4 + i) * Mtot + j];
       if (c.p > nt.p || (c.p == nt.p && c.idx < nt.idx)) nt = c;
     }
     tail[t] = nt;
@@ -640,10 +647,15 @@ cudaError_t launch_fill_partial(PeakPartial *partial, size_t n, cudaStream_t st)
 cudaError_t launch_finalize(const PeakPartial *partial, int n_det, int Mtot, int n_tt, float threshold,
                             lloid_peak *peaks, long long *n0, int B, PeakPartial *tail, const PeakPartial *tail_partial, int overlap,
                             cudaStream_t st) {
-  int g = 1;
-  while (g < n_tt && g < 32) g <<= 1;
-  const long long n = (long long)n_det * Mtot * g;
-  finalize_kernel<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(partial, n_det, Mtot, n_tt, g, threshold, peaks, n0, B, tail, tail_partial, overlap);
+  const long long n = (long long)n_det * Mtot;
+  int g = 1;                                                  // threads per (detector, template) pair: up to 8 while the grid is small
+  while (g < 8 && 2 * g <= n_tt && n * g < 148LL * 2048) g <<= 1;
+  const int tpb = 256 / g;
+  const unsigned grid = (unsigned)((n + tpb - 1) / tpb);
+  if (g == 1) finalize_kernel<1><<<grid, 256, 0, st>>>(partial, n_det, Mtot, n_tt, threshold, peaks, n0, B, tail, tail_partial, overlap);
+  else if (g == 2) finalize_kernel<2><<<grid, 256, 0, st>>>(partial, n_det, Mtot, n_tt, threshold, peaks, n0, B, tail, tail_partial, overlap);
+  else if (g == 4) finalize_kernel<4><<<grid, 256, 0, st>>>(partial, n_det, Mtot, n_tt, threshold, peaks, n0, B, tail, tail_partial, overlap);
+  else finalize_kernel<8><<<grid, 256, 0, st>>>(partial, n_det, Mtot, n_tt, threshold, peaks, n0, B, tail, tail_partial, overlap);
   return cudaGetLastError();
 }
 

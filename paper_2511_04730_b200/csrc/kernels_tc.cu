@@ -378,7 +378,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           }
           best.p = best.re * best.re + best.im * best.im;
         }
-        partial[((size_t)det * Mtot + tmpl_off + m) * n_tt + tl.slot * 4 + cs] = best;
+        partial[((size_t)det * n_tt + tl.slot * 4 + cs) * Mtot + tmpl_off + m] = best;   // [detector][slot][template]: a warp writes 512 contiguous bytes
       }
       }
     }
