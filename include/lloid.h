@@ -141,6 +141,19 @@ int lloid_stream_events(lloid_stream *stream, const lloid_peak *peaks, const int
 int lloid_svd_slice(const double *H, int32_t n_rows, int32_t n_taps, double energy, int32_t max_basis, int32_t *n_basis_out,
                     float *basis_out, float *recon_out, double *singular_out, double *kept_energy_out, void *cuda_stream);
 
+/* The same decomposition for callers that may not allocate device memory (a tight serving loop, a harness that forbids
+ * cudaMalloc): calls no cudaMalloc / cudaFree or allocating library routine.  The working set lives in a fixed device array
+ * inside the library (2.13 MiB, held by every GPU that loads the library until exit), hence the limits
+ *   n_rows <= 128 and n_taps <= 2048   (LLOID_SVD_NOALLOC_MAX_ROWS / _TAPS; larger -> EINVAL, use lloid_svd_slice)
+ * and H must be a DEVICE pointer (a host pointer is rejected with EINVAL: no staging buffer exists).  All other arguments,
+ * the results and the error codes are those of lloid_svd_slice (never ENOMEM).  Synchronous.  Every call on a device shares
+ * the array: calls that overlap on one GPU (two streams, two host threads) race and return garbage -- serialise them. */
+#define LLOID_SVD_NOALLOC_MAX_ROWS 128
+#define LLOID_SVD_NOALLOC_MAX_TAPS 2048
+int lloid_svd_slice_noalloc(const double *H, int32_t n_rows, int32_t n_taps, double energy, int32_t max_basis,
+                            int32_t *n_basis_out, float *basis_out, float *recon_out, double *singular_out,
+                            double *kept_energy_out, void *cuda_stream);
+
 /* xi^2 in the stream (Eq. 10).  lloid_bank_set_autocorrelation attaches the bank's template
  * autocorrelations (before lloid_stream_create): acorr [n_templates][2*delta+1][2] fp32 (re, im), host or device, R_j(t) for
  * t = -delta..delta with R_j(0) = 1 (definition below).  When EVERY bank of a stream carries autocorrelations of one delta

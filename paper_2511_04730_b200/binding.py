@@ -65,6 +65,7 @@ def _load():
         "lloid_bank_set_autocorrelation": (C.c_int, [vp, vp, i32]),
         "lloid_stream_xi2": (C.c_int, [vp, vp]),
         "lloid_svd_slice": (C.c_int, [vp, i32, i32, C.c_double, i32, C.POINTER(i32), vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]),
+        "lloid_svd_slice_noalloc": (C.c_int, [vp, i32, i32, C.c_double, i32, C.POINTER(i32), vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]),
         "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
@@ -85,7 +86,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_svd_slice", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_svd_slice", "lloid_svd_slice_noalloc", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
            "lloid_whitener_destroy", "lloid_whitener_hop_in", "lloid_whitener_hop_out", "lloid_whitener_psd_bins", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
@@ -193,6 +194,19 @@ def lloid_svd_slice(H: np.ndarray, energy: float = 0.9999, max_basis: Optional[i
                                 sig.ctypes.data_as(C.POINTER(C.c_double)), C.byref(kept), torch.cuda.current_stream(dev).cuda_stream))
     L = L.value
     return (U.flatten()[:L * N].reshape(L, N).cpu().numpy(), R.flatten()[:n * L].reshape(n, L).cpu().numpy(), sig[:L].copy(), kept.value)
+
+
+def lloid_svd_slice_noalloc(H_dev, energy: float, U_dev, R_dev, stream: int = 0):
+    """lloid_svd_slice without device allocations inside the library: H_dev float64 [n][N], U_dev float32 [max_basis][N] and
+    R_dev float32 [n][max_basis] are torch CUDA tensors the CALLER owns (n <= 128, N <= 2048).  Returns (L, sigma [L], kept
+    energy); U_dev / R_dev hold U [L][N] and R [n][L] compactly."""
+    n, N = H_dev.shape
+    mb = U_dev.shape[0]
+    L, kept = C.c_int32(), C.c_double()
+    sig = np.zeros(mb)
+    _check(_lib.lloid_svd_slice_noalloc(H_dev.data_ptr(), n, N, energy, mb, C.byref(L), U_dev.data_ptr(), R_dev.data_ptr(),
+                                        sig.ctypes.data_as(C.POINTER(C.c_double)), C.byref(kept), stream))
+    return L.value, sig[:L.value].copy(), kept.value
 
 
 def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):

@@ -108,6 +108,7 @@ def test_null_and_state_errors_without_a_device(lib):
         assert L.lloid_whitener_create(C.byref(w), *bad, None) == lib.LLOID_EINVAL and "whitener_create" in lib.lloid_last_error()
     n = C.c_int32()
     assert L.lloid_svd_slice(None, 4, 4, 0.9999, 4, C.byref(n), None, None, None, None, None) == lib.LLOID_EINVAL
+    assert L.lloid_svd_slice_noalloc(None, 4, 4, 0.9999, 4, C.byref(n), None, None, None, None, None) == lib.LLOID_EINVAL
     assert L.lloid_whitener_hop_in(None) == -1
 
 
