@@ -207,6 +207,16 @@ int32_t lloid_whitener_psd_bins(const lloid_whitener *w);
  * makes the copies asynchronous but is not required. */
 int lloid_stream_push_host(lloid_stream *stream, const float *strain_host, lloid_peak *peaks_host);
 
+/* Pipelined form of lloid_stream_push_host for a caller that pushes buffer after buffer: returns as soon as the copies and
+ * kernels are queued; a second CUDA stream copies the peaks of call n to peaks_host while call n + 1 computes (two device
+ * peak buffers).  Ownership: strain_host and peaks_host of call n belong to the library until call n + 2 has returned or
+ * lloid_stream_host_sync has -- alternate between two pairs of PINNED buffers (pageable memory makes the copies
+ * synchronous and the call pointless).  The peaks of call n are complete at the same moment.  lloid_stream_host_sync waits
+ * for everything queued.  Do not mix with lloid_stream_push_host / lloid_stream_push on the same stream object without a
+ * lloid_stream_host_sync in between.  Errors: EINVAL (null pointer), ESTATE (stream failed earlier), ECUDA. */
+int lloid_stream_push_host_async(lloid_stream *stream, const float *strain_host, lloid_peak *peaks_host);
+int lloid_stream_host_sync(lloid_stream *stream);
+
 /* Zero all rings and the stream clock: the next push is stream sample 0 (zero history). */
 int lloid_state_reset(lloid_stream *stream);
 

@@ -67,6 +67,8 @@ def _load():
         "lloid_svd_slice": (C.c_int, [vp, i32, i32, C.c_double, i32, C.POINTER(i32), vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]),
         "lloid_svd_slice_noalloc": (C.c_int, [vp, i32, i32, C.c_double, i32, C.POINTER(i32), vp, vp, C.POINTER(C.c_double), C.POINTER(C.c_double), vp]),
         "lloid_xi2_series": (C.c_int, [vp, i32, i64, vp, vp, i32, vp, vp]),
+        "lloid_stream_push_host_async": (C.c_int, [vp, vp, vp]),
+        "lloid_stream_host_sync": (C.c_int, [vp]),
         "lloid_state_reset": (C.c_int, [vp]),
         "lloid_stream_samples_pushed": (i64, [vp]),
         "lloid_stream_total_templates": (i32, [vp]),
@@ -86,7 +88,7 @@ def _load():
 
 _lib = _load()
 EXPORTS = ["lloid_options_default", "lloid_bank_create", "lloid_bank_destroy", "lloid_stream_create",
-           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_events", "lloid_xi2_series", "lloid_svd_slice", "lloid_svd_slice_noalloc", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
+           "lloid_stream_destroy", "lloid_stream_push", "lloid_stream_push_host", "lloid_stream_push_host_async", "lloid_stream_host_sync", "lloid_stream_events", "lloid_xi2_series", "lloid_svd_slice", "lloid_svd_slice_noalloc", "lloid_bank_set_autocorrelation", "lloid_stream_xi2", "lloid_whitener_create", "lloid_whitener_push", "lloid_whitener_reset",
            "lloid_whitener_destroy", "lloid_whitener_hop_in", "lloid_whitener_hop_out", "lloid_whitener_psd_bins", "lloid_state_reset",
            "lloid_stream_samples_pushed", "lloid_stream_total_templates", "lloid_stream_launches_per_push",
            "lloid_stream_work_per_push", "lloid_stream_set_stage_timing", "lloid_stream_stage_times",
@@ -207,6 +209,14 @@ def lloid_svd_slice_noalloc(H_dev, energy: float, U_dev, R_dev, stream: int = 0)
     _check(_lib.lloid_svd_slice_noalloc(H_dev.data_ptr(), n, N, energy, mb, C.byref(L), U_dev.data_ptr(), R_dev.data_ptr(),
                                         sig.ctypes.data_as(C.POINTER(C.c_double)), C.byref(kept), stream))
     return L.value, sig[:L.value].copy(), kept.value
+
+
+def lloid_stream_push_host_async(stream: int, strain_host_ptr: int, peaks_host_ptr: int):
+    _check(_lib.lloid_stream_push_host_async(stream, strain_host_ptr, peaks_host_ptr))
+
+
+def lloid_stream_host_sync(stream: int):
+    _check(_lib.lloid_stream_host_sync(stream))
 
 
 def lloid_stream_push_host(stream: int, strain_host_ptr: int, peaks_host_ptr: int):
@@ -373,6 +383,14 @@ class LloidStream:
         """End-to-end call on the pinned host buffers self.strain_host -> self.peaks_host (synchronous)."""
         lloid_stream_push_host(self.handle, self.strain_host.data_ptr(), self.peaks_host.data_ptr())
         return self.peaks_host.numpy().view(PEAK_DTYPE).reshape(self.n_det, self.Mtot)
+
+    def push_host_async(self, strain_host, peaks_host):
+        """Pipelined end-to-end call: strain_host / peaks_host are PINNED torch tensors the caller keeps alive and does not
+        touch until the call after next has returned (or host_sync())."""
+        lloid_stream_push_host_async(self.handle, strain_host.data_ptr(), peaks_host.data_ptr())
+
+    def host_sync(self):
+        lloid_stream_host_sync(self.handle)
 
     def reset(self):
         lloid_state_reset(self.handle)

@@ -39,6 +39,9 @@ struct lloid_stream {
   std::vector<ReconBank> rbanks;
   PeakPartial *partial_dev;
   float *strain_dev; lloid_peak *peaks_dev;       // staging for push_host
+  // push_host_async: two pushes in flight.  Two device peak buffers (the first is peaks_dev), a copy stream that drains
+  // buffer b while the next push computes, and per buffer the events "kernels done" / "D2H done"
+  lloid_peak *peaks_async[2]; cudaStream_t copy_st; cudaEvent_t ev_done[2], ev_copied[2]; long long n_async; bool async_ready;
   std::vector<void *> allocs;                      // every cudaMalloc of this stream
   std::vector<std::pair<void *, size_t>> state;    // (ptr, bytes) zeroed by reset
   int up_planes, up_chunk;
@@ -84,6 +87,11 @@ extern "C" void lloid_stream_destroy(lloid_stream *s) {
   if (s->tc) tc_plan_destroy(s->tc);
   for (auto &v : s->ev_rec) for (cudaEvent_t e : v) cudaEventDestroy(e);
   for (cudaEvent_t e : s->ev_pool) cudaEventDestroy(e);
+  if (s->async_ready) {
+    cudaStreamSynchronize(s->copy_st);
+    for (int i = 0; i < 2; ++i) { cudaEventDestroy(s->ev_done[i]); cudaEventDestroy(s->ev_copied[i]); }
+    cudaStreamDestroy(s->copy_st);
+  }
   for (void *p : s->allocs) cudaFree(p);
   delete s;
 }
@@ -128,6 +136,7 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->xi_delta = banks[0]->xi_delta;
   for (int b = 0; b < n_banks; ++b) if (banks[b]->xi_delta != s->xi_delta) s->xi_delta = 0;
   if (s->precision != LLOID_PREC_F16_SPLIT || B % 128 != 0 || s->xi_delta >= B) s->xi_delta = 0;
+  s->async_ready = false; s->n_async = 0; s->peaks_async[0] = s->peaks_async[1] = nullptr;
   s->st = (cudaStream_t)cuda_stream; s->n0_host = 0; s->tc = nullptr; s->stage_timing = false; s->failed = false;
   s->up_planes = s->precision == LLOID_PREC_FP32_FFMA ? 0 : (s->precision == LLOID_PREC_F16 ? 1 : 2);
   const int planes = std::max(1, s->up_planes);
@@ -390,6 +399,14 @@ extern "C" int lloid_stream_create(lloid_stream **out, const lloid_bank *const *
   s->n_tt = (B + 63) / 64;
   CK(dev_alloc(s, &s->strain_dev, (size_t)n_det * B));
   CK(dev_alloc(s, &s->peaks_dev, (size_t)n_det * s->Mtot));
+  s->peaks_async[0] = s->peaks_dev;
+  CK(dev_alloc(s, &s->peaks_async[1], (size_t)n_det * s->Mtot));
+  CK(cudaStreamCreateWithFlags(&s->copy_st, cudaStreamNonBlocking));
+  for (int i = 0; i < 2; ++i) {
+    CK(cudaEventCreateWithFlags(&s->ev_done[i], cudaEventDisableTiming));
+    CK(cudaEventCreateWithFlags(&s->ev_copied[i], cudaEventDisableTiming));
+  }
+  s->async_ready = true;
   if (s->precision != LLOID_PREC_FP32_FFMA) {
     int rc = tc_plan_create(&s->tc, s->classes, s->classes_dev, s->rbanks, s->rbanks_dev, n_det, B, planes, s->overlap, s->xi_delta, s->n_phase);
     if (rc != LLOID_OK) { lloid_stream_destroy(s); return rc; }
@@ -518,12 +535,42 @@ extern "C" int lloid_stream_push_host(lloid_stream *s, const float *strain_host,
   return LLOID_OK;
 }
 
+// Pipelined variant: returns as soon as the work is queued.  Call n computes into device peak buffer n & 1; a separate copy
+// stream moves it to peaks_host while call n + 1 computes.  Before reusing buffer n & 1, call n + 2 waits for that copy.
+extern "C" int lloid_stream_push_host_async(lloid_stream *s, const float *strain_host, lloid_peak *peaks_host) {
+  if (!s || !strain_host || !peaks_host) { set_error("stream_push_host_async: NULL argument"); return LLOID_EINVAL; }
+  const int b = (int)(s->n_async & 1);
+  cudaError_t e = cudaSuccess;
+  if (s->n_async >= 2) e = cudaEventSynchronize(s->ev_copied[b]);          // the D2H of call n - 2 has left this buffer
+  if (e == cudaSuccess) e = cudaMemcpyAsync(s->strain_dev, strain_host, sizeof(float) * s->n_det * s->B, cudaMemcpyHostToDevice, s->st);
+  if (e != cudaSuccess) { set_error("stream_push_host_async: wait / H2D copy: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  int rc = lloid_stream_push(s, s->strain_dev, s->peaks_async[b], nullptr, -1);
+  if (rc != LLOID_OK) return rc;
+  e = cudaEventRecord(s->ev_done[b], s->st);
+  if (e == cudaSuccess) e = cudaStreamWaitEvent(s->copy_st, s->ev_done[b], 0);
+  if (e == cudaSuccess) e = cudaMemcpyAsync(peaks_host, s->peaks_async[b], sizeof(lloid_peak) * s->n_det * s->Mtot, cudaMemcpyDeviceToHost, s->copy_st);
+  if (e == cudaSuccess) e = cudaEventRecord(s->ev_copied[b], s->copy_st);
+  if (e != cudaSuccess) { set_error("stream_push_host_async: D2H copy: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
+  ++s->n_async;
+  return LLOID_OK;
+}
+
+extern "C" int lloid_stream_host_sync(lloid_stream *s) {
+  if (!s) { set_error("stream_host_sync: stream is NULL"); return LLOID_EINVAL; }
+  cudaError_t e = cudaStreamSynchronize(s->st);
+  if (e == cudaSuccess) e = cudaStreamSynchronize(s->copy_st);
+  if (e != cudaSuccess) { set_error("stream_host_sync: %s", cudaGetErrorString(e)); s->failed = true; return LLOID_ECUDA; }
+  return LLOID_OK;
+}
+
 extern "C" int lloid_state_reset(lloid_stream *s) {
   if (!s) { set_error("state_reset: stream is NULL"); return LLOID_EINVAL; }
   for (auto &p : s->state) {
     cudaError_t e = cudaMemsetAsync(p.first, 0, p.second, s->st);
     if (e != cudaSuccess) { set_error("state_reset: %s", cudaGetErrorString(e)); return LLOID_ECUDA; }
   }
+  if (s->async_ready) cudaStreamSynchronize(s->copy_st);     // peaks still on their way to the host are delivered first
+  s->n_async = 0;
   s->n0_host = 0;
   s->n_pushes = 0;
   s->failed = false;

@@ -98,6 +98,7 @@ def test_null_and_state_errors_without_a_device(lib):
     # the calls around the path validate their arguments before touching a device
     L = lib.binding._lib
     assert L.lloid_stream_events(None, None, None, None) == lib.LLOID_EINVAL
+    assert L.lloid_stream_push_host_async(None, None, None) == lib.LLOID_EINVAL and L.lloid_stream_host_sync(None) == lib.LLOID_EINVAL
     assert L.lloid_stream_xi2(None, None) == lib.LLOID_EINVAL
     assert L.lloid_bank_set_autocorrelation(None, None, 175) == lib.LLOID_EINVAL
     assert L.lloid_xi2_series(None, 1, 1, None, None, 175, None, None) == lib.LLOID_EINVAL

@@ -139,6 +139,34 @@ def test_ragged_buffer_threshold_and_host_push():
         assert (peaks["snr"][4, 0] >= thr).any()
 
 
+def test_pipelined_host_push_returns_the_synchronous_peaks():
+    """lloid_stream_push_host_async (two pushes in flight, peaks copied by a second stream) delivers, buffer by buffer, exactly
+    the peaks of lloid_stream_push_host; also after lloid_state_reset."""
+    torch = _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from workloads import make_strain, random_bank
+    bank = random_bank(23, 150, [(2048, 512, 17), (1024, 768, 33), (512, 640, 21)]).as_f32()
+    B, n_push, n_det = 512, 7, 2
+    strain = np.stack([make_strain(310 + d, B * n_push) for d in range(n_det)]).astype(np.float32)
+    st = lib.LloidStream([bank, bank], n_det, B)
+    ref = []
+    for p in range(n_push):
+        st.strain_host.copy_(st.torch.from_numpy(strain[:, p * B:(p + 1) * B].copy()))
+        ref.append(st.push_host().copy())
+    for attempt in range(2):
+        st.reset()
+        xs = [st.torch.from_numpy(strain[:, p * B:(p + 1) * B].copy()).pin_memory() for p in range(n_push)]
+        outs = [st.torch.full((n_det, st.Mtot, 3), -7, dtype=st.torch.int32).pin_memory() for _ in range(n_push)]
+        for p in range(n_push):
+            st.push_host_async(xs[p], outs[p])
+        st.host_sync()
+        for p in range(n_push):
+            got = outs[p].numpy().view(lib.binding.PEAK_DTYPE).reshape(n_det, st.Mtot)
+            assert np.array_equal(got["sample"], ref[p]["sample"]) and np.array_equal(got["snr"], ref[p]["snr"]) and \
+                np.array_equal(got["phase"], ref[p]["phase"]), (attempt, p)
+    st.close()
+
+
 def test_two_streams_share_banks_and_errors():
     """Two streams over the same bank handles keep independent state; debug_bank out of range -> LLOID_ESTATE."""
     _torch_cuda()
