@@ -272,6 +272,24 @@ def test_degenerate_sizes(precision):
         check_peaks(peaks[:, det, :], ref, B, TOL[precision])
 
 
+@pytest.mark.parametrize("B", [32, 160])
+def test_short_and_odd_buffers_multirate(B):
+    """Buffers shorter than one 64-sample row block of the upsampled-Y planes (B = 32) and not a multiple of it (B = 160: a full
+    128-sample tile plus a ragged one whose second TMA box lies past the row pitch), three rates, two detectors, split mode."""
+    _torch_cuda()
+    from oracle import lloid_snr
+    from workloads import make_strain, random_bank
+    bank = random_bank(71, 37, [(2048, 256, 9), (1024, 384, 14), (512, 320, 11)]).as_f32()
+    n_push = 1920 // B
+    strain = np.stack([make_strain(710 + d, B * n_push) for d in range(2)])
+    rho_gpu, peaks = run_gpu([bank], strain, B, 2)
+    for det in range(2):
+        ref = lloid_snr(bank, strain[det])
+        emax, _ = check_snr(rho_gpu[det], ref, TOL[2])
+        assert emax <= TOL[2]
+        check_peaks(peaks[:, det, :], ref, B, TOL[2])
+
+
 def test_threshold_mismatch_is_rejected():
     """All banks of a stream share one trigger threshold (include/lloid.h): mixing thresholds is LLOID_EINVAL."""
     _torch_cuda()
