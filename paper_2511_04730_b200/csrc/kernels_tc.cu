@@ -657,7 +657,10 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
 struct TcPlan {
   int planes, n_det, B, n_tt;
   TcReconBank *rbanks_dev; TcReconTile *rtiles_dev; int n_rtiles;
-  TcReconTile *res_items_dev; int *res_begin_dev; int n_res_items, res_grid, res_ring_off, res_stages, str_stages;   // resident-R a3
+  // resident-R a3: up to 3 launches, the banks grouped by the size of their R tile, so that small-K banks get the deep operand
+  // ring their small resident region leaves room for (one launch sized for Kpad = 144 gave every bank 3 stages)
+  TcReconTile *res_items_dev[3]; int *res_begin_dev[3]; int n_res[3], res_grid[3], res_ring_off[3], res_stages[3], n_res_classes;
+  int n_res_items, str_stages;
   TcReconTile *tail_dev; int *tail_begin_dev; int n_tail, tail_grid, tail_tmin;   // tail pass of overlapped trigger windows
   TcReconTile *xi_dev; int *xi_begin_dev; int n_xi, xi_grid;   // xi^2 pass
   int *rbegin_dev, *cbegin_dev;
@@ -835,7 +838,6 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   cudaGetDevice(&dev);
   cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev);
   long long n_mu = 0, n_bm = 0;
-  int res_kmax = 0;
   for (size_t b = 0; b < banks.size(); ++b) {
     const ReconBank &k = banks[b];
     memset(&rb[b], 0, sizeof(TcReconBank));
@@ -859,7 +861,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     // resident R pays when the item reuses it over enough tiles (short buffers, config 4, stream R with Y instead)
     is_res[b] = (planes == 2 && k.Kpad <= RES_KMAX && (long long)n_det * ((B + TILE_N - 1) / TILE_N) >= 8) ? 1 : 0;
     const long long mt = (k.M + TILE_M - 1) / TILE_M;
-    if (is_res[b]) { n_bm += mt; res_kmax = std::max(res_kmax, k.Kpad); }
+    if (is_res[b]) n_bm += mt;
     else n_mu += mt * n_det;
   }
   const int nt = recon_run_tiles(B, n_mu), ntile = (B + TILE_N - 1) / TILE_N;
@@ -907,9 +909,38 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   p->n_tail = (int)tail.size();
   p->tail_grid = std::max(1, std::min(p->n_tail, sms));
   p->n_res_items = (int)ri.size();
-  p->res_grid = std::max(1, std::min(p->n_res_items, sms));
-  p->res_ring_off = ((res_kmax + RBK_RES - 1) / RBK_RES) * 4 * TILE_M * RBK_RES * 2;
-  p->res_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off) / (2 * TILE_M * RBK_RES * 2));
+  // classes by K blocks of the R tile: <= 2 (64 KB resident, 8 stages), 3 (96 KB, 7 stages), more (up to 160 KB, 3 stages);
+  // a class too small to fill the persistent grid joins its neighbour
+  std::vector<TcReconTile> rcls[3];
+  int rk[3] = {0, 0, 0};
+  for (const TcReconTile &t : ri) {
+    const int nkb = (rb[t.bank].Kpad + RBK_RES - 1) / RBK_RES, c = nkb <= 2 ? 0 : (nkb == 3 ? 1 : 2);
+    rcls[c].push_back(t); rk[c] = std::max(rk[c], rb[t.bank].Kpad);
+  }
+  for (int c = 0; c < 3; ++c) {
+    if (rcls[c].empty() || (long long)rcls[c].size() >= 4LL * sms) continue;
+    int d = -1;
+    for (int j = c + 1; j < 3 && d < 0; ++j) if (!rcls[j].empty()) d = j;
+    for (int j = c - 1; j >= 0 && d < 0; --j) if (!rcls[j].empty()) d = j;
+    if (d < 0) continue;                                         // the only class
+    rcls[d].insert(rcls[d].end(), rcls[c].begin(), rcls[c].end()); rk[d] = std::max(rk[d], rk[c]);
+    rcls[c].clear(); rk[c] = 0;
+  }
+  p->n_res_classes = 0;
+  std::vector<int> ibegin[3];
+  for (int c = 0; c < 3; ++c) {
+    if (rcls[c].empty()) continue;
+    const int i = p->n_res_classes++;
+    p->n_res[i] = (int)rcls[c].size();
+    p->res_grid[i] = std::max(1, std::min(p->n_res[i], sms));
+    p->res_ring_off[i] = ((rk[c] + RBK_RES - 1) / RBK_RES) * 4 * TILE_M * RBK_RES * 2;
+    p->res_stages[i] = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off[i]) / (2 * TILE_M * RBK_RES * 2));
+    // cost in cycles: 4 MMAs of ~97 cycles per 16 of K per tile (at least the epilogue's ~600), plus the once-per-item R load
+    lpt_assign(rcls[c], p->res_grid[i], [&](const TcReconTile &t) {
+      const long long kp = rb[t.bank].Kpad;
+      return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 388, 600) + 3000 + kp * 8; }, ibegin[i]);
+    if (!plan_upload(p, &p->res_items_dev[i], rcls[c]) || !plan_upload(p, &p->res_begin_dev[i], ibegin[i])) { tc_plan_destroy(p); return LLOID_ENOMEM; }
+  }
   p->str_stages = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES) / (3 * planes * TILE_M * RBK_STR * 2));
   p->n_rtiles = (int)rt.size();
   p->recon_grid = std::max(1, std::min(p->n_rtiles, sms));
@@ -931,16 +962,11 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     cu.swap(all);
   }
   lpt_assign(rt, p->recon_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, rbegin);
-  std::vector<int> ibegin;
-  // cost in cycles: 4 MMAs of ~97 cycles per 16 of K per tile (at least the epilogue's ~600), plus the once-per-item R load
-  lpt_assign(ri, p->res_grid, [&](const TcReconTile &t) {
-    const long long kp = rb[t.bank].Kpad;
-    return (long long)t.ndet * t.nt * std::max<long long>(kp / 16 * 388, 600) + 3000 + kp * 8; }, ibegin);
   std::vector<int> tbegin, xbegin;
   lpt_assign(xit, p->xi_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, xbegin);
   lpt_assign(tail, p->tail_grid, [&](const TcReconTile &t) { return (long long)t.nt * (rb[t.bank].Kpad / 16 + 2); }, tbegin);
-  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) || !plan_upload(p, &p->res_items_dev, ri) ||
-      !plan_upload(p, &p->res_begin_dev, ibegin) || !plan_upload(p, &p->tail_dev, tail) || !plan_upload(p, &p->tail_begin_dev, tbegin) ||
+  if (!plan_upload(p, &p->cbegin_dev, cbegin) || !plan_upload(p, &p->rbegin_dev, rbegin) ||
+      !plan_upload(p, &p->tail_dev, tail) || !plan_upload(p, &p->tail_begin_dev, tbegin) ||
       !plan_upload(p, &p->xi_dev, xit) || !plan_upload(p, &p->xi_begin_dev, xbegin)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
   if (!plan_upload(p, &p->cmaps_dev, cm) || !plan_upload(p, &p->cunits_dev, cu) || !plan_upload(p, &p->rbanks_dev, rb) ||
       !plan_upload(p, &p->rtiles_dev, rt)) { tc_plan_destroy(p); return LLOID_ENOMEM; }
@@ -973,7 +999,7 @@ cudaError_t tc_launch_corr(TcPlan *p, const long long *n0, cudaStream_t st, int 
 }
 
 int tc_plan_n_tt(const TcPlan *p) { return p->n_tt; }
-int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + (p->n_res_items ? 1 : 0) + (p->n_tail ? 1 : 0); }
+int tc_plan_recon_launches(const TcPlan *p) { return (p->n_rtiles ? 1 : 0) + p->n_res_classes + (p->n_tail ? 1 : 0); }
 
 cudaError_t tc_launch_xi2(TcPlan *p, const lloid_peak *peaks, float *xi_partial, int Mtot, int row_base, cudaStream_t st) {
   if (p->n_xi == 0 || p->planes != 2) return cudaErrorInvalidValue;
@@ -996,9 +1022,9 @@ cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot,
 }
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
-  if (p->n_res_items) {
-    recon_tc_kernel<2, true><<<p->res_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->res_items_dev, p->res_begin_dev, p->n_det, p->B,
-                                                                              partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off, p->res_stages, 0);
+  for (int i = 0; i < p->n_res_classes; ++i) {
+    recon_tc_kernel<2, true><<<p->res_grid[i], RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->res_items_dev[i], p->res_begin_dev[i], p->n_det, p->B,
+                                                                                 partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off[i], p->res_stages[i], 0);
     cudaError_t e0 = cudaGetLastError();
     if (e0 != cudaSuccess) return e0;
   }
