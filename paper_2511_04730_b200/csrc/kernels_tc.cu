@@ -661,6 +661,9 @@ struct TcPlan {
   // ring their small resident region leaves room for (one launch sized for Kpad = 144 gave every bank 3 stages)
   TcReconTile *res_items_dev[3]; int *res_begin_dev[3]; int n_res[3], res_grid[3], res_ring_off[3], res_stages[3], n_res_classes;
   int n_res_items, str_stages;
+  // the a3 launches of one push are independent (disjoint partial-peak slots): all but the first go to side streams between a
+  // fork and a join event, so that the CTAs of the next launch fill the SMs the previous one's tail leaves idle
+  cudaStream_t side[3]; cudaEvent_t fork_ev, join_ev[3]; bool side_ready;
   TcReconTile *tail_dev; int *tail_begin_dev; int n_tail, tail_grid, tail_tmin;   // tail pass of overlapped trigger windows
   TcReconTile *xi_dev; int *xi_begin_dev; int n_xi, xi_grid;   // xi^2 pass
   int *rbegin_dev, *cbegin_dev;
@@ -777,6 +780,10 @@ static bool plan_upload(TcPlan *p, T **dst, const std::vector<T> &h) {
 
 void tc_plan_destroy(TcPlan *p) {
   if (!p) return;
+  if (p->side_ready) {
+    cudaEventDestroy(p->fork_ev);
+    for (int i = 0; i < 3; ++i) { cudaStreamSynchronize(p->side[i]); cudaEventDestroy(p->join_ev[i]); cudaStreamDestroy(p->side[i]); }
+  }
   for (void *q : p->allocs) cudaFree(q);
   delete p;
 }
@@ -786,6 +793,14 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   *out = nullptr;
   TcPlan *p = new TcPlan();
   p->planes = planes; p->n_det = n_det; p->B = B; p->classes_dev = classes_dev;
+  {
+    bool ok = cudaEventCreateWithFlags(&p->fork_ev, cudaEventDisableTiming) == cudaSuccess;
+    for (int i = 0; i < 3 && ok; ++i)
+      ok = cudaStreamCreateWithFlags(&p->side[i], cudaStreamNonBlocking) == cudaSuccess &&
+           cudaEventCreateWithFlags(&p->join_ev[i], cudaEventDisableTiming) == cudaSuccess;
+    if (!ok) { set_error("stream_create: cannot create the side streams / events of a3"); delete p; return LLOID_ECUDA; }
+    p->side_ready = true;
+  }
   // ---- a2: one tensor map per class; units = (row tile, tap segment, group of <= 4 (detector, column tile) sub-tiles),
   //      dealt to the persistent CTAs in order of decreasing cost
   std::vector<TcCorrClass> cm(classes.size());
@@ -1022,20 +1037,37 @@ cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot,
 }
 
 cudaError_t tc_launch_recon(TcPlan *p, PeakPartial *partial, int Mtot, float *snr_debug, int debug_bank, cudaStream_t st) {
-  for (int i = 0; i < p->n_res_classes; ++i) {
-    recon_tc_kernel<2, true><<<p->res_grid[i], RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->res_items_dev[i], p->res_begin_dev[i], p->n_det, p->B,
-                                                                                 partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off[i], p->res_stages[i], 0);
-    cudaError_t e0 = cudaGetLastError();
-    if (e0 != cudaSuccess) return e0;
+  // launch k = 0 on the caller's stream, k >= 1 on side stream k - 1 (after the fork event); the caller's stream then waits for all
+  const int n_launch = p->n_res_classes + (p->n_rtiles ? 1 : 0);
+  cudaError_t e = cudaSuccess;
+  if (n_launch > 1) e = cudaEventRecord(p->fork_ev, st);
+  int k = 0;
+  auto stream_of = [&](int i) -> cudaStream_t {
+    if (i == 0) return st;
+    cudaStreamWaitEvent(p->side[i - 1], p->fork_ev, 0);
+    return p->side[i - 1];
+  };
+  for (int i = 0; i < p->n_res_classes && e == cudaSuccess; ++i, ++k) {
+    recon_tc_kernel<2, true><<<p->res_grid[i], RECON_THREADS, p->recon_smem, stream_of(k)>>>(p->rbanks_dev, p->res_items_dev[i], p->res_begin_dev[i], p->n_det, p->B,
+                                                                                         partial, Mtot, p->n_tt, snr_debug, debug_bank, p->res_ring_off[i], p->res_stages[i], 0);
+    e = cudaGetLastError();
   }
-  if (p->n_rtiles == 0) return cudaSuccess;
-  if (p->planes == 2)
-    recon_tc_kernel<2, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
-  else
-    recon_tc_kernel<1, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, st>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
-                                                                                partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
-  return cudaGetLastError();
+  if (p->n_rtiles && e == cudaSuccess) {
+    cudaStream_t s2 = stream_of(k++);
+    if (p->planes == 2)
+      recon_tc_kernel<2, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, s2>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
+                                                                                  partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
+    else
+      recon_tc_kernel<1, false><<<p->recon_grid, RECON_THREADS, p->recon_smem, s2>>>(p->rbanks_dev, p->rtiles_dev, p->rbegin_dev, p->n_det, p->B,
+                                                                                  partial, Mtot, p->n_tt, snr_debug, debug_bank, 0, p->str_stages, 0);
+    e = cudaGetLastError();
+  }
+  for (int i = 1; i < k; ++i) {                                   // join (also after a failed launch: nothing may be left dangling)
+    cudaError_t e2 = cudaEventRecord(p->join_ev[i - 1], p->side[i - 1]);
+    if (e2 == cudaSuccess) e2 = cudaStreamWaitEvent(st, p->join_ev[i - 1], 0);
+    if (e == cudaSuccess) e = e2;
+  }
+  return e;
 }
 
 }  // namespace lloid
