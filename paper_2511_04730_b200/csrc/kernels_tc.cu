@@ -1024,7 +1024,7 @@ cudaError_t tc_launch_xi2(TcPlan *p, const lloid_peak *peaks, float *xi_partial,
   return cudaGetLastError();
 }
 
-// tail pass: the peak of every template over the buffer's last `overlap` samples -> tail_partial [n_det][Mtot][4]
+// tail pass: the peak of every template over the buffer's last `overlap` samples -> tail_partial [n_det][4][Mtot]
 cudaError_t tc_launch_recon_tail(TcPlan *p, PeakPartial *tail_partial, int Mtot, cudaStream_t st) {
   if (p->n_tail == 0) return cudaSuccess;
   if (p->planes == 2)

@@ -37,7 +37,7 @@ struct lloid_stream {
   float *uptaps_dev; int *uptap_off_dev;
   ReconBank *rbanks_dev;
   std::vector<ReconBank> rbanks;
-  PeakPartial *partial_dev;
+  PeakPartial *partial_dev;                        // [n_det][n_tt][Mtot] partial peaks (slot-major)
   float *strain_dev; lloid_peak *peaks_dev;       // staging for push_host
   // push_host_async: two pushes in flight.  Two device peak buffers (the first is peaks_dev), a copy stream that drains
   // buffer b while the next push computes, and per buffer the events "kernels done" / "D2H done"
