@@ -280,11 +280,15 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           __syncwarp();
           if (lane == 0) mbar_arrive(&tempty[buf]);
           if (has && tbase + 31 >= k0 - delta && tbase <= k0 + delta) {
+            // sample i of the slice is autocorrelation lag u0 + i: one base pointer, constant offsets, and the window as a range
+            // of i (no per-sample index arithmetic); the pointer is only dereferenced inside the row
+            const int u0 = tbase - k0 + delta;
+            const int i_lo = max(0, -u0), i_hi = min(32, 2 * delta + 1 - u0);
+            const float2 *Rp = reinterpret_cast<const float2 *>(reinterpret_cast<const char *>(R) + (long long)u0 * (long long)sizeof(float2));
 #pragma unroll
             for (int i = 0; i < 32; ++i) {
-              const int u = tbase + i - k0 + delta;
-              if (u >= 0 && u <= 2 * delta) {
-                const float2 a = R[u];
+              if (i >= i_lo && i < i_hi) {
+                const float2 a = __ldg(Rp + i);
                 const float dr = __uint_as_float(vr[i]) - (z0r * a.x - z0i * a.y), di = __uint_as_float(vi[i]) - (z0r * a.y + z0i * a.x);
                 num = fmaf(dr, dr, fmaf(di, di, num));
               }
