@@ -247,6 +247,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     const int q = warp & 3, cs = (warp - 2) >> 2, etid = threadIdx.x - 64;
     const uint32_t lane_base = (uint32_t)(q * 32) << 16;
     float4 *rec_re = rec + etid, *rec_im = rec + (PK_CHUNK / 4) * EPI_THREADS + etid;   // conflict-free 16-byte slots
+    const uint32_t rec_re_s = smem_u32(rec_re), rec_im_s = smem_u32(rec_im);
     int it = 0;
     for (int ti = i_begin; ti < i_end; ++ti) {
       const TcReconTile tl = tiles[ti];
@@ -343,8 +344,9 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
 #pragma unroll
               for (int j = 0; j < PK_CHUNK / 4; ++j) {  // the loaded registers are consecutive: plain 16-byte stores
                 const int o = c * PK_CHUNK + 4 * j;
-                rec_re[j * EPI_THREADS] = make_float4(__uint_as_float(vr[o]), __uint_as_float(vr[o + 1]), __uint_as_float(vr[o + 2]), __uint_as_float(vr[o + 3]));
-                rec_im[j * EPI_THREADS] = make_float4(__uint_as_float(vi[o]), __uint_as_float(vi[o + 1]), __uint_as_float(vi[o + 2]), __uint_as_float(vi[o + 3]));
+                // explicit st.shared (through the generic pointer the compiler emits generic stores)
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(rec_re_s + j * EPI_THREADS * 16), "r"(vr[o]), "r"(vr[o + 1]), "r"(vr[o + 2]), "r"(vr[o + 3]) : "memory");
+                asm volatile("st.shared.v4.b32 [%0], {%1, %2, %3, %4};" ::"r"(rec_im_s + j * EPI_THREADS * 16), "r"(vi[o]), "r"(vi[o + 1]), "r"(vi[o + 2]), "r"(vi[o + 3]) : "memory");
               }
             }
           }
