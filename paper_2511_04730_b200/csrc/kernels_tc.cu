@@ -85,7 +85,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
   constexpr int STAGE_BYTES = NT * RTILE_BYTES;
   const int STAGES = n_stages;                                  // <= RMAX_STAGES; the resident region [0, ring_off) comes first
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned; stays a shared-space pointer
   uint8_t *ring = smem + ring_off;
   float4 *rec = (float4 *)(ring + STAGES * STAGE_BYTES);       // [re, im][PK_CHUNK / 4][EPI_THREADS] float4
   uint64_t *bars = (uint64_t *)((uint8_t *)rec + REC_BYTES);
@@ -432,7 +432,7 @@ corr_tc_kernel(const CorrClass *__restrict__ classes, const TcCorrClass *__restr
   constexpr int STAGES = PLANES == 2 ? 4 : 6;
   constexpr int STAGE_BYTES = PLANES * TILE_BYTES;
   extern __shared__ __align__(1024) uint8_t smem_raw[];
-  uint8_t *smem = (uint8_t *)(((uintptr_t)smem_raw + 1023) & ~(uintptr_t)1023);
+  uint8_t *smem = smem_raw + ((1024u - (smem_u32(smem_raw) & 1023u)) & 1023u);   // 1024-byte aligned; stays a shared-space pointer
   uint8_t *strips = smem + STAGES * STAGE_BYTES;                 // [2 buffers][PLANES][STRIP_PLANE]
   float *xwin = (float *)(strips + 2 * PLANES * STRIP_PLANE);    // [XWIN_TOTAL]
   uint64_t *bars = (uint64_t *)(xwin + XWIN_TOTAL);
