@@ -167,6 +167,41 @@ def test_pipelined_host_push_returns_the_synchronous_peaks():
     st.close()
 
 
+def test_mixed_bank_sizes_are_deterministic_and_match_single_bank_streams():
+    """Banks of very different basis counts in one stream take every a3 route at once (three resident launches by R size, the
+    streaming variant, the tail pass, all but one on side streams): the peaks are bit-identical from run to run and equal to
+    those of each bank filtered alone."""
+    torch = _torch_cuda()
+    import paper_2511_04730_b200 as lib
+    from workloads import make_strain, random_bank
+    shapes = [[(2048, 1024, 4), (1024, 1024, 4), (512, 1024, 4), (256, 1152, 4)],                                  # K = 16
+              [(2048, 1024, 16), (1024, 1024, 16), (512, 1024, 16), (256, 1152, 16), (128, 1024, 16)],             # K = 80
+              [(2048, 1024, 20), (1024, 1024, 30), (512, 2048, 40), (256, 3072, 50)],                              # K = 140
+              [(2048, 1024, 16), (1024, 1024, 16), (512, 2048, 32), (256, 3072, 64), (128, 4096, 64)]]             # K = 192: streaming
+    banks = [random_bank(300 + i, 1000 if i < 4 else 777, shapes[i % 4]).as_f32() for i in range(8)]
+    B, n_push, n_det = 2048, 5, 3
+    strain = np.stack([make_strain(900 + d, B * n_push) for d in range(n_det)]).astype(np.float32)
+    many = [banks[i % 8] for i in range(480)]                       # >= 4 x 148 items per group keeps the groups apart
+    st = lib.LloidStream(many, n_det, B, trigger_overlap=200)
+    assert st.launches_per_push >= 9                                # 4 + three resident groups + streaming + tail
+    runs = []
+    for attempt in range(2):
+        st.reset()
+        runs.append([st.push(strain[:, p * B:(p + 1) * B]).copy() for p in range(n_push)])
+    st.close()
+    off = np.concatenate([[0], np.cumsum([b.M for b in many])])
+    for p in range(n_push):
+        assert runs[0][p].tobytes() == runs[1][p].tobytes(), p
+    for i in (0, 1, 2, 3):
+        one = lib.LloidStream([banks[i]], n_det, B, trigger_overlap=200)
+        for p in range(n_push):
+            pk = one.push(strain[:, p * B:(p + 1) * B])
+            for j in (i, i + 8 * 59):                                # the first and the last copy of this bank in the big stream
+                got = runs[0][p][:, off[j]:off[j + 1]]
+                assert np.array_equal(got["sample"], pk["sample"]) and np.array_equal(got["snr"], pk["snr"]), (i, j, p)
+        one.close()
+
+
 def test_two_streams_share_banks_and_errors():
     """Two streams over the same bank handles keep independent state; debug_bank out of range -> LLOID_ESTATE."""
     _torch_cuda()
