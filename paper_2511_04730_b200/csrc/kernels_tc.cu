@@ -32,15 +32,16 @@ static constexpr int TILE_M = 128;           // rows of U / templates of R per t
 static constexpr int TILE_N = 128;           // max columns (time samples) per tile
 static constexpr int BK = 64;                // K elements per TMA box = one 128-byte swizzled row of fp16
 static constexpr int TILE_BYTES = TILE_M * BK * 2;   // 16 KB
+static constexpr int RSTEP_BYTES = 4 * 128 * 16 * 2;   // a3 resident variant: R of ONE K step (16 of K): [Rre, Rim, Rre corr, Rim corr] x 128 rows x 32 B
 static constexpr int RBK_RES = 32;           // a3 resident variant: K elements per TMA box (64-byte swizzled rows)
 static constexpr int RBK_STR = 64;           // a3 streaming variant: 128-byte swizzled rows (fewer barrier round trips per K)
-static constexpr int RES_KMAX = 144;         // resident-R variant: the item's R tile (4 tiles x ceil(Kpad / 32) K blocks) <= 160 KB
+static constexpr int RES_KMAX = 144;         // resident-R variant: the item's R tile (Kpad / 16 K steps of 16 KB) <= 144 KB
 static constexpr int RMAX_STAGES = 8;        // a3 operand ring: at most 8 stages
 static constexpr int RECON_SMEM_BUDGET = 232448 - 1024 - 256;   // dynamic shared memory per CTA minus alignment and barriers
 
 struct TcReconTile { int bank, det, ndet, m0, t0, nt, slot; };   // detectors det..det+ndet-1 x nt consecutive time tiles from sample t0; partial slot
 struct TcReconBank {                         // device copy, 64-byte aligned (CUtensorMap needs it)
-  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 32 x 128, 64-byte swizzle (resident variant)
+  CUtensorMap mapR;                          // [planes*2*Mpad rows][Kpad] fp16, box 16 x 128, 32-byte swizzle (resident variant: one K step per box)
   CUtensorMap mapR64;                        // the same array, box 64 x 128, 128-byte swizzle (streaming variant)
   // upsampled Y, sample-contiguous rows: plane 0 fp16 [n_det*Kpad rows][Bp], boxes of 64 samples x
   // 32 / 64 rows; correction plane bytes [n_det*2*Kpad rows][Bp], boxes of 128 samples x 64 / 128 rows; 128-byte swizzle
@@ -116,10 +117,13 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
         const int nkb = (bk->Kpad + RBK - 1) / RBK;
         if (RES) {
           if (ti > i_begin) mbar_wait(rfree, (uint32_t)(ti - i_begin - 1) & 1);    // the previous item's MMAs have read R
-          mbar_arrive_expect_tx(rfull, nkb * 4 * RTILE_BYTES);
-          for (int kb = 0; kb < nkb; ++kb)
+          // resident R: one 16 KB group per K step of 16 (Kpad / 16 groups: no padding to the 32-row Y blocks, which leaves the
+          // ring one more stage at Kpad = 144)
+          const int nst = bk->Kpad / 16;
+          mbar_arrive_expect_tx(rfull, nst * RSTEP_BYTES);
+          for (int ks = 0; ks < nst; ++ks)
 #pragma unroll
-            for (int j = 0; j < 4; ++j) tma_load_2d(smem + (kb * 4 + j) * RTILE_BYTES, &bk->mapR, rfull, kb * RBK, j * bk->Mpad + tl.m0);
+            for (int j = 0; j < 4; ++j) tma_load_2d(smem + ks * RSTEP_BYTES + j * (RSTEP_BYTES / 4), &bk->mapR, rfull, ks * 16, j * bk->Mpad + tl.m0);
         }
         for (int d = 0; d < tl.ndet; ++d)
         for (int tt = 0; tt < tl.nt; ++tt) {
@@ -169,7 +173,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
     constexpr uint32_t T16 = RTILE_BYTES >> 4;                    // operand tile size in 16-byte descriptor units
     constexpr uint32_t YK16 = 2048 >> 4, YK8 = 4096 >> 4;          // one MMA of K: 16 fp16 rows / 32 byte rows of 128 B
     int stage = 0; uint32_t phase = 0; int it = 0;
-    const uint64_t ring_d = desc_kmajor_sw(smem_u32(ring), RBK), res_d = desc_kmajor_sw(smem_u32(smem), RBK);
+    const uint64_t ring_d = desc_kmajor_sw(smem_u32(ring), RBK), res_d = desc_kmajor_sw(smem_u32(smem), 16);
     const uint64_t ring_y16 = desc_mnmajor_sw128(smem_u32(ring), RTILE_BYTES / 2), ring_y8 = desc_mnmajor_sw128(smem_u32(ring), 16);
     for (int ti = i_begin; ti < i_end; ++ti) {
       const TcReconTile tl = tiles[ti];
@@ -201,7 +205,7 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
           // base descriptors; every operand tile / K step is a constant added to the 16-byte address field
           const uint64_t sd = ring_d + (uint64_t)(stage * (STAGE_BYTES >> 4));
           const uint64_t sy16 = ring_y16 + (uint64_t)(stage * (STAGE_BYTES >> 4)), sy8 = ring_y8 + (uint64_t)(stage * (STAGE_BYTES >> 4));
-          const uint64_t rd = RES ? res_d + (uint64_t)(kb * 4 * T16) : sd;
+          const uint64_t rd = RES ? res_d + (uint64_t)(kb * 2 * (RSTEP_BYTES >> 4)) : sd;   // two K steps per Y block
           const int nk = min(RBK / 16, (Kpad - kb * RBK) / 16);    // K is padded to 16: the last box may be partly zero fill
           if (elect_one()) {
 #pragma unroll
@@ -210,10 +214,11 @@ recon_tc_kernel(const TcReconBank *__restrict__ banks, const TcReconTile *__rest
               const bool acc = (kb | k) != 0;
               if (RES) {
                 const uint64_t y_hi = sy16 + YK16 * k, y_8 = sy8 + (T16 + YK8 * k);
-                mma_f16_ss(d_re, rd + (0 * T16 + 2 * k), y_hi, idesc, acc);
-                mma_f16_ss(d_im, rd + (1 * T16 + 2 * k), y_hi, idesc, acc);
-                mma_f8_ss(d_re, rd + (2 * T16 + 2 * k), y_8, idesc8, true);
-                mma_f8_ss(d_im, rd + (3 * T16 + 2 * k), y_8, idesc8, true);
+                constexpr uint32_t RS = RSTEP_BYTES >> 4, RP = RS / 4;   // K step and plane strides of the resident R, 16-byte units
+                mma_f16_ss(d_re, rd + (k * RS + 0 * RP), y_hi, idesc, acc);
+                mma_f16_ss(d_im, rd + (k * RS + 1 * RP), y_hi, idesc, acc);
+                mma_f8_ss(d_re, rd + (k * RS + 2 * RP), y_8, idesc8, true);
+                mma_f8_ss(d_im, rd + (k * RS + 3 * RP), y_8, idesc8, true);
               } else {
                 const uint64_t y_hi = sy16 + (2 * T16 + YK16 * k);
                 mma_f16_ss(d_re, sd + (0 * T16 + 2 * k), y_hi, idesc, acc);
@@ -864,7 +869,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     memset(&rb[b], 0, sizeof(TcReconBank));
     const uint64_t Bp = (uint64_t)yup_pitch(B), yrows = (uint64_t)n_det * k.Kpad;
     const uint8_t *y8 = reinterpret_cast<const uint8_t *>(k.yup) + 2 * k.yup_plane_stride;      // the correction plane (bytes)
-    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_RES) ||
+    if (!make_map(&rb[b].mapR, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, 16) ||
         !make_map(&rb[b].mapR64, k.R16, (uint64_t)planes * 2 * k.Mpad, (uint64_t)k.Kpad, TILE_M, RBK_STR) ||
         !make_map_y(&rb[b].mapY, k.yup, false, yrows, Bp, RBK_RES) || !make_map_y(&rb[b].mapY64, k.yup, false, yrows, Bp, RBK_STR)) {
       tc_plan_destroy(p); return LLOID_ECUDA;
@@ -930,7 +935,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
   p->n_tail = (int)tail.size();
   p->tail_grid = std::max(1, std::min(p->n_tail, sms));
   p->n_res_items = (int)ri.size();
-  // classes by K blocks of the R tile: <= 2 (64 KB resident, 8 stages), 3 (96 KB, 7 stages), more (up to 160 KB, 3 stages);
+  // classes by K blocks of the R tile: <= 2 (<= 64 KB resident, 8 stages), 3 (<= 96 KB, 7-8 stages), more (<= 144 KB, 4 stages);
   // a class too small to fill the persistent grid joins its neighbour
   std::vector<TcReconTile> rcls[3];
   int rk[3] = {0, 0, 0};
@@ -954,7 +959,7 @@ int tc_plan_create(TcPlan **out, const std::vector<CorrClass> &classes, const Co
     const int i = p->n_res_classes++;
     p->n_res[i] = (int)rcls[c].size();
     p->res_grid[i] = std::max(1, std::min(p->n_res[i], sms));
-    p->res_ring_off[i] = ((rk[c] + RBK_RES - 1) / RBK_RES) * 4 * TILE_M * RBK_RES * 2;
+    p->res_ring_off[i] = (rk[c] / 16) * RSTEP_BYTES;
     p->res_stages[i] = std::min(RMAX_STAGES, (RECON_SMEM_BUDGET - REC_BYTES - p->res_ring_off[i]) / (2 * TILE_M * RBK_RES * 2));
     // cost in cycles: 4 MMAs of ~97 cycles per 16 of K per tile (at least the epilogue's ~600), plus the once-per-item R load
     lpt_assign(rcls[c], p->res_grid[i], [&](const TcReconTile &t) {
