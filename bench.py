@@ -422,6 +422,14 @@ def measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, K, W,
     ms = [a.elapsed_time(b) for a, b in zip(ev0, ev1)]
     t_dev = max_over_ranks(sum(ms) / 1e3, dev, world)
 
+    # ---- per-stage device times (CUDA events recorded by the library on its stream) for the roofline: K more steps right
+    #      after the timed ones (later in the run the board approaches its power cap and the stages would read slower)
+    st.set_stage_timing(True)
+    for i in range(K):
+        flush(); st.push_device(pool[step]); step += 1
+    n_cov, stage_ms = st.stage_times()
+    st.set_stage_timing(False)
+
     # ---- end to end through the C ABI with HOST buffers (pinned): H2D strain + push + D2H peaks per step
     t_e2e = 0.0
     for i in range(K):
@@ -471,12 +479,6 @@ def measure_config(lib, torch, dist, dev, local_rank, rank, world, cfg_no, K, W,
         g1.record(); torch.cuda.synchronize()
         ev_ms = g0.elapsed_time(g1) / 5
 
-    # ---- per-stage device times (CUDA events recorded by the library on its stream) for the roofline
-    st.set_stage_timing(True)
-    for i in range(K):
-        flush(); st.push_device(pool[step]); step += 1
-    n_cov, stage_ms = st.stage_times()
-    st.set_stage_timing(False)
     launches = st.launches_per_push
     d2h = int(st.peaks_host.numel() * st.peaks_host.element_size())
     handles, Ms = st.release_banks() if shared is None else (None, None)      # the caller owns (and frees) the bank handles
